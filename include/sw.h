@@ -1,0 +1,133 @@
+/*
+ * sw.h -- C ABI of libsw.so: the Swendsen-Wang multi-cluster sweep of a 2D periodic L x L lattice
+ * (q-state Potts; q-state clock through Wolff's embedded cluster) on one NVIDIA B200 (sm_100a).
+ *
+ * Source of the semantics: arXiv 1202.0635 (Komura & Okabe), /root/reference/PAPER.md:
+ *   Potts Hamiltonian  H = -J sum_<ij> (delta(S_i,S_j) - 1), periodic            PAPER.md:25-30 eq.(1)
+ *   one sweep = bond activation -> cluster labeling -> new state per cluster
+ *   proper label of a cluster = its smallest label
+ *   clock Hamiltonian  H = -J sum_<ij> S_i . S_j, theta = 2 pi p / q              PAPER.md:132-136 eq.(4)
+ *   embedded cluster (Wolff) for the clock model
+ *   measurement of energy and magnetisation, M^2 of eq.(3)
+ * Everything the paper leaves open (random-number keying, thresholds, clock reflection rule, order
+ * of operations) is fixed in DESIGN.md section 3, readings R1..R14.
+ *
+ * General rules
+ *   - J = 1.  Site i = y*L + x (x fastest).  Site i owns the bonds to (x+1 mod L, y) [direction 0]
+ *     and (x, y+1 mod L) [direction 1].  Spin values are 0..q-1, one uint8 per site, row-major.
+ *   - Every function returning int returns SW_OK (0) or a negative SW_ERR_* code; the two
+ *     constructors return a pointer or NULL.  After a failure sw_last_error() describes it.
+ *     No exception crosses the boundary.  A context is not thread-safe.
+ *   - "host" pointers are ordinary CPU memory owned by the caller; "device" pointers are CUDA
+ *     device memory of the current device.  The library never frees caller memory.
+ *   - All work of a context is enqueued on its stream.  Functions are synchronous at return
+ *     (the stream is synchronised) unless the name ends in _async.
+ *   - There is no CPU fallback: if no CUDA device is usable every call fails with SW_ERR_CUDA.
+ */
+#ifndef SW_H_
+#define SW_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sw_ctx sw_ctx; /* opaque, owned by the library */
+
+enum { SW_POTTS = 0, SW_CLOCK = 1 };
+enum { SW_OK = 0, SW_ERR_ARG = -1, SW_ERR_CUDA = -2, SW_ERR_NOMEM = -3, SW_ERR_UNSUPPORTED = -4 };
+
+/* Labeling back-ends (sw_set_algorithm).  Every back-end produces the same spins bit for bit. */
+enum {
+    SW_ALGO_AUTO = 0,    /* tiled when L allows it, else generic */
+    SW_ALGO_GENERIC = 1, /* whole-lattice union-find in global memory; any L >= 2 */
+    SW_ALGO_TILED = 2    /* tile-local union-find in shared memory + boundary merge; needs L % 128 == 0 */
+};
+
+/* Limits of the GPU path: 2 <= L <= 16384 (site index must leave 4 spare bits in an int32 label),
+ * 2 <= q <= 16, T finite and > 0, model in {SW_POTTS, SW_CLOCK}.  Violations: NULL / SW_ERR_ARG. */
+#define SW_MAX_L 16384
+#define SW_MAX_Q 16
+
+/* Bytes of device workspace sw_create_in() needs for this problem (0 if the arguments are invalid). */
+size_t sw_workspace_bytes(int L, int q, int model);
+
+/* Create a context; the initial configuration S^0 is drawn from the INIT stream of `seed`
+ * (R12) and the sweep index is 0.  sw_create allocates its own device memory and stream.
+ * sw_create_in uses caller-owned device memory `d_workspace` (>= sw_workspace_bytes, 256-byte
+ * aligned, must outlive the context) and the caller's CUDA stream handle `cuda_stream`
+ * (a cudaStream_t cast to void*; NULL = the legacy default stream).  Returns NULL on failure. */
+sw_ctx *sw_create(int L, int q, int model, double T, uint64_t seed);
+sw_ctx *sw_create_in(int L, int q, int model, double T, uint64_t seed,
+                     void *d_workspace, size_t bytes, void *cuda_stream);
+
+/* Destroy a context (NULL is a no-op).  Caller-owned workspace/stream are left untouched. */
+void sw_destroy(sw_ctx *ctx);
+
+/* n >= 0 full SW sweeps (steps S0-S4 of DESIGN.md section 1), sweep indices
+ * t .. t+n-1 where t = sw_sweep_index().  sw_sweep(a); sw_sweep(b) == sw_sweep(a+b).
+ * sw_sweep returns after the work is complete; sw_sweep_async only enqueues it on the stream. */
+int sw_sweep(sw_ctx *ctx, int n);
+int sw_sweep_async(sw_ctx *ctx, int n);
+int sw_sync(sw_ctx *ctx);
+
+/* n sweeps with the observables of every configuration recorded ("+ measurement"):
+ * row k (q entries) of each HOST output = bond_hist / state_hist of the configuration BEFORE the
+ * k-th sweep of this call (R10).  Outputs hold n*q int64 each. */
+int sw_sweep_record(sw_ctx *ctx, int n, int64_t *bond_hist_out, int64_t *state_hist_out);
+
+/* Observables of the current configuration, HOST outputs of q int64 each (R11):
+ * bond_hist[d] = #{owned bonds with (S_i - S_nbr) mod q == d};  state_hist[k] = #{S_i == k}.
+ * Potts energy E/J = 2*L*L - bond_hist[0]; M^2 from state_hist by eq.(3). */
+int sw_observables(sw_ctx *ctx, int64_t *bond_hist, int64_t *state_hist);
+
+/* Copy the configuration to / from HOST memory (L*L bytes, row-major, values 0..q-1).
+ * sw_set_spins also sets the absolute sweep index (resume / oracle hand-off); values >= q are
+ * rejected with SW_ERR_ARG and leave the context unchanged. */
+int sw_get_spins(sw_ctx *ctx, uint8_t *host_out);
+int sw_set_spins(sw_ctx *ctx, const uint8_t *host_in, uint64_t sweep_index);
+uint64_t sw_sweep_index(sw_ctx *ctx); /* 0 for NULL */
+
+/* The integer bond thresholds in use (R6): Potts -> 1 word, clock -> (2q)^2 words,
+ * table[ci*2q + cj].  `out` (HOST) may be NULL to query `count` only. */
+int sw_get_thresholds(sw_ctx *ctx, uint32_t *out, int *count);
+
+/* Debug exports (HOST outputs).  sw_get_labels: canonical root (minimum site index of the cluster)
+ * of every site for the LAST executed sweep, L*L int32 (SW_ERR_ARG before any sweep).
+ * sw_debug_bonds: the bonds sweep t = sw_sweep_index() would activate on the current configuration,
+ * L*L bytes, bit0 = +x, bit1 = +y; does not advance the state. */
+int sw_get_labels(sw_ctx *ctx, int32_t *host_out);
+int sw_debug_bonds(sw_ctx *ctx, uint8_t *host_out);
+
+/* Choose the labeling back-end (SW_ALGO_*); SW_ERR_UNSUPPORTED if L does not allow it. */
+int sw_set_algorithm(sw_ctx *ctx, int algo);
+int sw_get_algorithm(sw_ctx *ctx); /* the back-end actually in use (never SW_ALGO_AUTO) */
+
+/* Labeling work counters accumulated since creation (the analogue of the paper's iteration counts,
+ * PAPER.md:75): out[0] = sweeps counted, out[1] = cross-tile merge attempts, out[2] = merge atomics
+ * that changed a root, out[3] = open tile roots processed by the flatten pass.  HOST output of 4 doubles;
+ * counters are only collected after sw_enable_stats(ctx, 1) (they cost atomics). */
+int sw_enable_stats(sw_ctx *ctx, int on);
+int sw_stats(sw_ctx *ctx, double *out4);
+
+/* n sweeps with every kernel bracketed by CUDA events on the context's stream (one stream sync per sweep, so
+ * this is a measurement mode, not the production path): ms_out[k] (HOST, SW_MAX_KERNELS doubles) receives the
+ * summed device time of kernel k over the n sweeps, *n_kernels the number of distinct kernels per sweep of the
+ * active back-end; sw_kernel_name(ctx, k) names them (static string, NULL if k is out of range).
+ * The configuration advances exactly as with sw_sweep(ctx, n). */
+#define SW_MAX_KERNELS 8
+int sw_sweep_profile(sw_ctx *ctx, int n, double *ms_out, int *n_kernels);
+const char *sw_kernel_name(sw_ctx *ctx, int k);
+
+/* Number of kernel launches this context has enqueued since creation. */
+uint64_t sw_launch_count(sw_ctx *ctx);
+
+/* Thread-local description of the last failure in this thread ("" if none). */
+const char *sw_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SW_H_ */

@@ -1,0 +1,491 @@
+// libsw.so -- C ABI of include/sw.h: context, host-side scheduling of the sweep kernels, copies.
+// All arithmetic of the method runs in the kernels of sw_generic.cuh / sw_tiled.cuh; the only host
+// arithmetic is the threshold table (double precision, once per context; R6/R7).
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "sw.h"
+#include "sw_generic.cuh"
+#include "sw_philox.cuh"
+#include "sw_tiled.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU_TRY(expr)                                                                              \
+    do {                                                                                          \
+        cudaError_t e_ = (expr);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(e_ == cudaErrorMemoryAllocation ? SW_ERR_NOMEM : SW_ERR_CUDA, "%s: %s",   \
+                        #expr, cudaGetErrorString(e_));                                           \
+    } while (0)
+
+constexpr size_t ALIGN = 1024;
+constexpr int REC_ROWS = 512;  // rows of the device ring used by sw_sweep_record
+constexpr int OBS_WORDS = 32;  // [0,16) bond_hist, [16,32) state_hist
+
+size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+bool args_ok(int L, int q, int model)
+{
+    return L >= 2 && L <= SW_MAX_L && q >= 2 && q <= SW_MAX_Q && (model == SW_POTTS || model == SW_CLOCK);
+}
+
+struct Carve {
+    size_t spins, labels, bonds, table, obs, flag, stats, ring, tiled, total;
+};
+
+Carve carve(int L, int q)
+{
+    (void)q;
+    const size_t N = (size_t)L * (size_t)L;
+    Carve c;
+    size_t off = 0;
+    c.spins = off;  off += align_up(N);
+    c.labels = off; off += align_up(4 * N);
+    c.bonds = off;  off += align_up(N);
+    c.table = off;  off += align_up(4 * (size_t)(2 * SW_MAX_Q) * (2 * SW_MAX_Q));
+    c.obs = off;    off += align_up(8 * OBS_WORDS);
+    c.flag = off;   off += align_up(64);
+    c.stats = off;  off += align_up(64);
+    c.ring = off;   off += align_up((size_t)REC_ROWS * OBS_WORDS * 8);
+    c.tiled = off;  off += align_up(sw::tiled_workspace_bytes(L));
+    c.total = off;
+    return c;
+}
+
+}  // namespace
+
+struct sw_ctx {
+    int L = 0, q = 0, model = 0;
+    double T = 0.0;
+    uint64_t seed = 0, t = 0;
+    size_t N = 0;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false, own_ws = false;
+    char *ws = nullptr;
+    Carve cv{};
+    uint8_t *spins = nullptr, *bonds = nullptr;
+    int32_t *labels = nullptr;
+    uint32_t *table = nullptr;
+    unsigned long long *obs = nullptr, *stats = nullptr, *ring = nullptr;
+    int *flag = nullptr;
+    char *tiled_ws = nullptr;
+    sw::Model md{};
+    sw::PhiloxKey key{};
+    std::vector<uint32_t> thr_host;  // 1 (Potts) or (2q)^2 (clock)
+    int algo = SW_ALGO_GENERIC;
+    bool have_labels = false, stats_on = false;
+    int last_algo = 0;
+    uint64_t launches = 0, stat_sweeps = 0;
+    sw::TiledState tiled{};
+};
+
+namespace {
+
+uint32_t thr_from_p(double p)
+{
+    double v = std::floor(p * 4294967296.0);
+    if (!(v > 0.0)) return 0u;
+    if (v >= 4294967295.0) return 0xFFFFFFFFu;
+    return (uint32_t)v;
+}
+
+// DESIGN.md R1 (Potts) and R4 (clock).  Host, double precision.
+void build_thresholds(sw_ctx *c)
+{
+    if (c->model == SW_POTTS) {
+        c->thr_host.assign(1, thr_from_p(1.0 - std::exp(-1.0 / c->T)));
+    } else {
+        const int n = 2 * c->q;
+        const double pi = 3.14159265358979323846;
+        c->thr_host.assign((size_t)n * n, 0u);
+        std::vector<double> s(n);
+        for (int k = 0; k < n; ++k) s[k] = (k % c->q == 0) ? 0.0 : std::sin(pi * (double)k / (double)c->q);
+        for (int a = 0; a < n; ++a)
+            for (int b = 0; b < n; ++b) {
+                const double pr = s[a] * s[b];
+                if (pr > 0.0) c->thr_host[(size_t)a * n + b] = thr_from_p(1.0 - std::exp(-2.0 * pr / c->T));
+            }
+    }
+}
+
+inline unsigned blocks_for(size_t n, unsigned bs) { return (unsigned)((n + bs - 1) / bs); }
+
+const char *const GENERIC_KERNELS[] = { "k_bonds", "k_label_init", "k_union", "k_flatten", "k_flip" };
+
+// ev (optional): ev[0] is recorded before the first kernel, ev[k+1] after kernel k.
+int generic_sweep(sw_ctx *c, uint32_t t, cudaEvent_t *ev)
+{
+    const unsigned bs = 256;
+    const uint32_t N = c->md.N;
+    if (ev) cudaEventRecord(ev[0], c->stream);
+    sw::k_bonds<<<blocks_for((N + 1) / 2, bs), bs, 0, c->stream>>>(c->md, c->key, t, c->spins, c->bonds);
+    if (ev) cudaEventRecord(ev[1], c->stream);
+    sw::k_label_init<<<blocks_for(N, bs), bs, 0, c->stream>>>(N, c->labels);
+    if (ev) cudaEventRecord(ev[2], c->stream);
+    sw::k_union<<<blocks_for(N, bs), bs, 0, c->stream>>>(c->md, c->bonds, c->labels);
+    if (ev) cudaEventRecord(ev[3], c->stream);
+    sw::k_flatten<<<blocks_for(N, bs), bs, 0, c->stream>>>(N, c->labels);
+    if (ev) cudaEventRecord(ev[4], c->stream);
+    sw::k_flip<<<blocks_for(N, bs), bs, 0, c->stream>>>(c->md, c->key, t, c->labels, c->spins);
+    if (ev) cudaEventRecord(ev[5], c->stream);
+    c->launches += 5;
+    return SW_OK;
+}
+
+int one_sweep(sw_ctx *c, cudaEvent_t *ev = nullptr)
+{
+    const uint32_t t = (uint32_t)c->t;
+    int rc;
+    if (c->algo == SW_ALGO_TILED) {
+        rc = sw::tiled_sweep(c->tiled, c->md, c->key, t, c->spins, c->labels, c->stream, c->stats_on ? c->stats : nullptr,
+                             &c->launches, ev);
+        if (rc != 0) return fail(SW_ERR_CUDA, "tiled sweep launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    } else {
+        rc = generic_sweep(c, t, ev);
+    }
+    c->last_algo = c->algo;
+    c->have_labels = true;
+    if (c->stats_on) c->stat_sweeps += 1;
+    c->t += 1;
+    return rc;
+}
+
+int launch_observables(sw_ctx *c, unsigned long long *dst)
+{
+    CU_TRY(cudaMemsetAsync(dst, 0, 8 * OBS_WORDS, c->stream));
+    const unsigned grid = (unsigned)std::min<size_t>((c->N + 255) / 256, 148 * 8);
+    sw::k_observables<<<grid, 256, 0, c->stream>>>(c->md, c->spins, dst);
+    c->launches += 1;
+    return SW_OK;
+}
+
+sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, size_t bytes, void *stream, bool own)
+{
+    if (!args_ok(L, q, model) || !(T > 0.0) || !std::isfinite(T)) {
+        fail(SW_ERR_ARG, "sw_create: need 2<=L<=%d, 2<=q<=%d, model in {0,1}, finite T>0 (got L=%d q=%d model=%d T=%g)",
+             SW_MAX_L, SW_MAX_Q, L, q, model, T);
+        return nullptr;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        fail(SW_ERR_CUDA, "sw_create: no usable CUDA device (this library has no CPU fallback)");
+        return nullptr;
+    }
+    sw_ctx *c = new (std::nothrow) sw_ctx();
+    if (!c) { fail(SW_ERR_NOMEM, "sw_create: out of host memory"); return nullptr; }
+    c->L = L; c->q = q; c->model = model; c->T = T; c->seed = seed; c->t = 0;
+    c->N = (size_t)L * (size_t)L;
+    c->cv = carve(L, q);
+    if (own) {
+        cudaError_t e = cudaMalloc((void **)&c->ws, c->cv.total);
+        if (e != cudaSuccess) {
+            fail(SW_ERR_NOMEM, "sw_create: cudaMalloc(%zu) failed: %s", c->cv.total, cudaGetErrorString(e));
+            delete c;
+            return nullptr;
+        }
+        c->own_ws = true;
+        e = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) {
+            fail(SW_ERR_CUDA, "sw_create: cudaStreamCreate failed: %s", cudaGetErrorString(e));
+            cudaFree(c->ws);
+            delete c;
+            return nullptr;
+        }
+        c->own_stream = true;
+    } else {
+        if (!ws || bytes < c->cv.total || ((uintptr_t)ws & 255u)) {
+            fail(SW_ERR_ARG, "sw_create_in: workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)",
+                 c->cv.total, bytes);
+            delete c;
+            return nullptr;
+        }
+        c->ws = (char *)ws;
+        c->stream = (cudaStream_t)stream;
+    }
+    c->spins = (uint8_t *)(c->ws + c->cv.spins);
+    c->labels = (int32_t *)(c->ws + c->cv.labels);
+    c->bonds = (uint8_t *)(c->ws + c->cv.bonds);
+    c->table = (uint32_t *)(c->ws + c->cv.table);
+    c->obs = (unsigned long long *)(c->ws + c->cv.obs);
+    c->flag = (int *)(c->ws + c->cv.flag);
+    c->stats = (unsigned long long *)(c->ws + c->cv.stats);
+    c->ring = (unsigned long long *)(c->ws + c->cv.ring);
+    c->tiled_ws = c->ws + c->cv.tiled;
+    c->key = sw::make_philox_key(seed);
+    build_thresholds(c);
+    c->md.L = L; c->md.q = q; c->md.model = model; c->md.N = (uint32_t)c->N;
+    c->md.thr_potts = (model == SW_POTTS) ? c->thr_host[0] : 0u;
+    c->md.table = c->table;
+
+    bool ok = true;
+    ok = ok && cudaMemsetAsync(c->table, 0, 4 * (size_t)(2 * SW_MAX_Q) * (2 * SW_MAX_Q), c->stream) == cudaSuccess;
+    if (model == SW_CLOCK)
+        ok = ok && cudaMemcpyAsync(c->table, c->thr_host.data(), 4 * c->thr_host.size(), cudaMemcpyHostToDevice, c->stream) == cudaSuccess;
+    ok = ok && cudaMemsetAsync(c->stats, 0, 64, c->stream) == cudaSuccess;
+    if (ok) {
+        sw::k_init_spins<<<blocks_for((c->N + 3) / 4, 256), 256, 0, c->stream>>>(c->md, c->key, c->spins);
+        c->launches += 1;
+        ok = cudaGetLastError() == cudaSuccess;
+    }
+    c->algo = sw::tiled_supported(L) ? SW_ALGO_TILED : SW_ALGO_GENERIC;
+    if (ok && sw::tiled_supported(L)) ok = sw::tiled_init(c->tiled, c->md, c->tiled_ws, c->spins, c->labels, c->stream) == 0;
+    ok = ok && cudaStreamSynchronize(c->stream) == cudaSuccess;
+    if (!ok) {
+        fail(SW_ERR_CUDA, "sw_create: device initialisation failed: %s", cudaGetErrorString(cudaGetLastError()));
+        sw_destroy(c);
+        return nullptr;
+    }
+    return c;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t sw_workspace_bytes(int L, int q, int model)
+{
+    if (!args_ok(L, q, model)) return 0;
+    return carve(L, q).total;
+}
+
+sw_ctx *sw_create(int L, int q, int model, double T, uint64_t seed)
+{
+    return create_impl(L, q, model, T, seed, nullptr, 0, nullptr, true);
+}
+
+sw_ctx *sw_create_in(int L, int q, int model, double T, uint64_t seed, void *d_workspace, size_t bytes, void *cuda_stream)
+{
+    return create_impl(L, q, model, T, seed, d_workspace, bytes, cuda_stream, false);
+}
+
+void sw_destroy(sw_ctx *c)
+{
+    if (!c) return;
+    if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
+    sw::tiled_destroy(c->tiled);
+    if (c->own_ws && c->ws) cudaFree(c->ws);
+    if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
+    delete c;
+}
+
+int sw_sweep_async(sw_ctx *c, int n)
+{
+    if (!c || n < 0) return fail(SW_ERR_ARG, "sw_sweep: NULL context or n < 0");
+    if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep: sweep index would exceed 2^32-1");
+    for (int k = 0; k < n; ++k) {
+        int rc = one_sweep(c);
+        if (rc != SW_OK) return rc;
+    }
+    CU_TRY(cudaGetLastError());
+    return SW_OK;
+}
+
+int sw_sync(sw_ctx *c)
+{
+    if (!c) return fail(SW_ERR_ARG, "sw_sync: NULL context");
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    return SW_OK;
+}
+
+int sw_sweep(sw_ctx *c, int n)
+{
+    int rc = sw_sweep_async(c, n);
+    if (rc != SW_OK) return rc;
+    return sw_sync(c);
+}
+
+int sw_sweep_record(sw_ctx *c, int n, int64_t *bond_out, int64_t *state_out)
+{
+    if (!c || n < 0 || !bond_out || !state_out) return fail(SW_ERR_ARG, "sw_sweep_record: bad arguments");
+    if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_record: sweep index would exceed 2^32-1");
+    std::vector<unsigned long long> host((size_t)REC_ROWS * OBS_WORDS);
+    int done = 0;
+    while (done < n) {
+        const int chunk = std::min(REC_ROWS, n - done);
+        for (int k = 0; k < chunk; ++k) {
+            int rc = launch_observables(c, c->ring + (size_t)k * OBS_WORDS);
+            if (rc != SW_OK) return rc;
+            rc = one_sweep(c);
+            if (rc != SW_OK) return rc;
+        }
+        CU_TRY(cudaGetLastError());
+        CU_TRY(cudaMemcpyAsync(host.data(), c->ring, (size_t)chunk * OBS_WORDS * 8, cudaMemcpyDeviceToHost, c->stream));
+        CU_TRY(cudaStreamSynchronize(c->stream));
+        for (int k = 0; k < chunk; ++k)
+            for (int j = 0; j < c->q; ++j) {
+                bond_out[(size_t)(done + k) * c->q + j] = (int64_t)host[(size_t)k * OBS_WORDS + j];
+                state_out[(size_t)(done + k) * c->q + j] = (int64_t)host[(size_t)k * OBS_WORDS + 16 + j];
+            }
+        done += chunk;
+    }
+    return SW_OK;
+}
+
+int sw_observables(sw_ctx *c, int64_t *bond_hist, int64_t *state_hist)
+{
+    if (!c || !bond_hist || !state_hist) return fail(SW_ERR_ARG, "sw_observables: NULL argument");
+    int rc = launch_observables(c, c->obs);
+    if (rc != SW_OK) return rc;
+    CU_TRY(cudaGetLastError());
+    unsigned long long host[OBS_WORDS];
+    CU_TRY(cudaMemcpyAsync(host, c->obs, sizeof(host), cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    for (int j = 0; j < c->q; ++j) {
+        bond_hist[j] = (int64_t)host[j];
+        state_hist[j] = (int64_t)host[16 + j];
+    }
+    return SW_OK;
+}
+
+int sw_get_spins(sw_ctx *c, uint8_t *host_out)
+{
+    if (!c || !host_out) return fail(SW_ERR_ARG, "sw_get_spins: NULL argument");
+    CU_TRY(cudaMemcpyAsync(host_out, c->spins, c->N, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    return SW_OK;
+}
+
+int sw_set_spins(sw_ctx *c, const uint8_t *host_in, uint64_t sweep_index)
+{
+    if (!c || !host_in) return fail(SW_ERR_ARG, "sw_set_spins: NULL argument");
+    if (sweep_index > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_set_spins: sweep index must fit 32 bits");
+    // Stage in the bond scratch buffer, validate on the device, then commit.
+    CU_TRY(cudaMemcpyAsync(c->bonds, host_in, c->N, cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(cudaMemsetAsync(c->flag, 0, sizeof(int), c->stream));
+    sw::k_check_spins<<<blocks_for(c->N, 256), 256, 0, c->stream>>>(c->md.N, (uint32_t)c->q, c->bonds, c->flag);
+    c->launches += 1;
+    CU_TRY(cudaGetLastError());
+    int bad = 0;
+    CU_TRY(cudaMemcpyAsync(&bad, c->flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    if (bad) return fail(SW_ERR_ARG, "sw_set_spins: a spin value is >= q = %d", c->q);
+    CU_TRY(cudaMemcpyAsync(c->spins, c->bonds, c->N, cudaMemcpyDeviceToDevice, c->stream));
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    c->t = sweep_index;
+    c->have_labels = false;
+    return SW_OK;
+}
+
+uint64_t sw_sweep_index(sw_ctx *c) { return c ? c->t : 0; }
+
+int sw_get_thresholds(sw_ctx *c, uint32_t *out, int *count)
+{
+    if (!c || !count) return fail(SW_ERR_ARG, "sw_get_thresholds: NULL argument");
+    *count = (int)c->thr_host.size();
+    if (out) std::memcpy(out, c->thr_host.data(), 4 * c->thr_host.size());
+    return SW_OK;
+}
+
+int sw_get_labels(sw_ctx *c, int32_t *host_out)
+{
+    if (!c || !host_out) return fail(SW_ERR_ARG, "sw_get_labels: NULL argument");
+    if (!c->have_labels) return fail(SW_ERR_ARG, "sw_get_labels: no sweep has been executed on this configuration");
+    const int32_t *src = c->labels;
+    if (c->last_algo == SW_ALGO_TILED) {
+        // The tiled back-end leaves tile roots in the label words; resolve them in place (idempotent).
+        int rc = sw::tiled_resolve_labels(c->tiled, c->md, c->labels, c->stream, &c->launches);
+        if (rc != 0) return fail(SW_ERR_CUDA, "sw_get_labels: resolve failed");
+    }
+    CU_TRY(cudaGetLastError());
+    CU_TRY(cudaMemcpyAsync(host_out, src, 4 * c->N, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    return SW_OK;
+}
+
+int sw_debug_bonds(sw_ctx *c, uint8_t *host_out)
+{
+    if (!c || !host_out) return fail(SW_ERR_ARG, "sw_debug_bonds: NULL argument");
+    sw::k_bonds<<<blocks_for((c->N + 1) / 2, 256), 256, 0, c->stream>>>(c->md, c->key, (uint32_t)c->t, c->spins, c->bonds);
+    c->launches += 1;
+    CU_TRY(cudaGetLastError());
+    CU_TRY(cudaMemcpyAsync(host_out, c->bonds, c->N, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    return SW_OK;
+}
+
+int sw_set_algorithm(sw_ctx *c, int algo)
+{
+    if (!c) return fail(SW_ERR_ARG, "sw_set_algorithm: NULL context");
+    if (algo == SW_ALGO_AUTO) algo = sw::tiled_supported(c->L) ? SW_ALGO_TILED : SW_ALGO_GENERIC;
+    if (algo == SW_ALGO_TILED && !sw::tiled_supported(c->L))
+        return fail(SW_ERR_UNSUPPORTED, "sw_set_algorithm: the tiled back-end needs L %% %d == 0 (L = %d)", sw::TILE_W, c->L);
+    if (algo != SW_ALGO_GENERIC && algo != SW_ALGO_TILED) return fail(SW_ERR_ARG, "sw_set_algorithm: unknown back-end %d", algo);
+    c->algo = algo;
+    return SW_OK;
+}
+
+int sw_get_algorithm(sw_ctx *c) { return c ? c->algo : SW_ERR_ARG; }
+
+int sw_enable_stats(sw_ctx *c, int on)
+{
+    if (!c) return fail(SW_ERR_ARG, "sw_enable_stats: NULL context");
+    c->stats_on = on != 0;
+    return SW_OK;
+}
+
+int sw_stats(sw_ctx *c, double *out4)
+{
+    if (!c || !out4) return fail(SW_ERR_ARG, "sw_stats: NULL argument");
+    unsigned long long h[4];
+    CU_TRY(cudaMemcpyAsync(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < 4; ++k) out4[k] = (double)h[k];
+    out4[0] = (double)c->stat_sweeps;
+    return SW_OK;
+}
+
+int sw_sweep_profile(sw_ctx *c, int n, double *ms_out, int *n_kernels)
+{
+    if (!c || n < 0 || !ms_out || !n_kernels) return fail(SW_ERR_ARG, "sw_sweep_profile: bad arguments");
+    if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_profile: sweep index would exceed 2^32-1");
+    const int nk = (c->algo == SW_ALGO_TILED) ? sw::TILED_NUM_KERNELS : 5;
+    cudaEvent_t ev[SW_MAX_KERNELS + 1];
+    for (int k = 0; k <= nk; ++k) CU_TRY(cudaEventCreate(&ev[k]));
+    for (int k = 0; k < SW_MAX_KERNELS; ++k) ms_out[k] = 0.0;
+    int rc = SW_OK;
+    for (int it = 0; it < n && rc == SW_OK; ++it) {
+        rc = one_sweep(c, ev);
+        if (rc != SW_OK) break;
+        if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = fail(SW_ERR_CUDA, "sw_sweep_profile: sync failed"); break; }
+        for (int k = 0; k < nk; ++k) {
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, ev[k], ev[k + 1]);
+            ms_out[k] += (double)ms;
+        }
+    }
+    for (int k = 0; k <= nk; ++k) cudaEventDestroy(ev[k]);
+    *n_kernels = nk;
+    return rc;
+}
+
+const char *sw_kernel_name(sw_ctx *c, int k)
+{
+    if (!c || k < 0) return nullptr;
+    if (c->algo == SW_ALGO_TILED) return k < sw::TILED_NUM_KERNELS ? sw::TILED_KERNELS[k] : nullptr;
+    return k < 5 ? GENERIC_KERNELS[k] : nullptr;
+}
+
+uint64_t sw_launch_count(sw_ctx *c) { return c ? c->launches : 0; }
+
+const char *sw_last_error(void) { return g_err; }
+
+}  // extern "C"
