@@ -89,11 +89,29 @@ __device__ __forceinline__ int32_t uf_find(const int32_t *lab, int32_t a)
     return a;
 }
 
+// find with path halving: every node passed on the way is re-pointed to its grandparent.  A racing atomicMin or
+// another halving store can only replace an ancestor by another ancestor, so connectivity is kept.  Loads may be
+// served by a stale L1 line: a stale parent is still an ancestor, and a stale "root" is caught by the atomicMin
+// of uf_union, which returns the true parent.  (L1-cached loads keep the hot roots of large clusters out of L2.)
+__device__ __forceinline__ int32_t uf_find_halve(int32_t *lab, int32_t a)
+{
+    int32_t cur = lab[a];
+    if (cur != a) {
+        int32_t prev = a, next;
+        while (cur > (next = lab[cur])) {
+            lab[prev] = next;
+            prev = cur;
+            cur = next;
+        }
+    }
+    return cur;
+}
+
 __device__ __forceinline__ void uf_union(int32_t *lab, int32_t a, int32_t b)
 {
     for (;;) {
-        a = uf_find(lab, a);
-        b = uf_find(lab, b);
+        a = uf_find_halve(lab, a);
+        b = uf_find_halve(lab, b);
         if (a == b) return;
         if (a < b) { const int32_t tmp = a; a = b; b = tmp; }
         const int32_t old = atomicMin(lab + a, b);  // a > b
