@@ -13,7 +13,7 @@
 #include "sw.h"
 #include "sw_generic.cuh"
 #include "sw_philox.cuh"
-#include "sw_tiled.cuh"
+#include "sw_tile.cuh"
 
 namespace {
 
@@ -247,7 +247,7 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
         ok = cudaGetLastError() == cudaSuccess;
     }
     c->algo = sw::tiled_supported(L) ? SW_ALGO_TILED : SW_ALGO_GENERIC;
-    if (ok && sw::tiled_supported(L)) ok = sw::tiled_init(c->tiled, c->md, c->tiled_ws, c->spins, c->labels, c->stream) == 0;
+    if (ok && sw::tiled_supported(L)) ok = sw::tiled_init(c->tiled, c->md, c->tiled_ws) == 0;
     ok = ok && cudaStreamSynchronize(c->stream) == cudaSuccess;
     if (!ok) {
         fail(SW_ERR_CUDA, "sw_create: device initialisation failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -281,7 +281,6 @@ void sw_destroy(sw_ctx *c)
 {
     if (!c) return;
     if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
-    sw::tiled_destroy(c->tiled);
     if (c->own_ws && c->ws) cudaFree(c->ws);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
     delete c;
@@ -399,14 +398,19 @@ int sw_get_labels(sw_ctx *c, int32_t *host_out)
 {
     if (!c || !host_out) return fail(SW_ERR_ARG, "sw_get_labels: NULL argument");
     if (!c->have_labels) return fail(SW_ERR_ARG, "sw_get_labels: no sweep has been executed on this configuration");
-    const int32_t *src = c->labels;
     if (c->last_algo == SW_ALGO_TILED) {
-        // The tiled back-end leaves tile roots in the label words; resolve them in place (idempotent).
-        int rc = sw::tiled_resolve_labels(c->tiled, c->md, c->labels, c->stream, &c->launches);
-        if (rc != 0) return fail(SW_ERR_CUDA, "sw_get_labels: resolve failed");
+        // The tiled back-end keeps tile-local labels + a sparse global parent array: resolve into a scratch buffer.
+        int32_t *tmp = nullptr;
+        CU_TRY(cudaMalloc((void **)&tmp, 4 * c->N));
+        int rc = sw::tiled_resolve_labels(c->tiled, c->md, c->labels, tmp, c->stream, &c->launches);
+        cudaError_t e = rc == 0 ? cudaMemcpyAsync(host_out, tmp, 4 * c->N, cudaMemcpyDeviceToHost, c->stream) : cudaErrorUnknown;
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        cudaFree(tmp);
+        if (e != cudaSuccess) return fail(SW_ERR_CUDA, "sw_get_labels: resolve failed: %s", cudaGetErrorString(cudaGetLastError()));
+        return SW_OK;
     }
     CU_TRY(cudaGetLastError());
-    CU_TRY(cudaMemcpyAsync(host_out, src, 4 * c->N, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(cudaMemcpyAsync(host_out, c->labels, 4 * c->N, cudaMemcpyDeviceToHost, c->stream));
     CU_TRY(cudaStreamSynchronize(c->stream));
     return SW_OK;
 }
@@ -427,7 +431,7 @@ int sw_set_algorithm(sw_ctx *c, int algo)
     if (!c) return fail(SW_ERR_ARG, "sw_set_algorithm: NULL context");
     if (algo == SW_ALGO_AUTO) algo = sw::tiled_supported(c->L) ? SW_ALGO_TILED : SW_ALGO_GENERIC;
     if (algo == SW_ALGO_TILED && !sw::tiled_supported(c->L))
-        return fail(SW_ERR_UNSUPPORTED, "sw_set_algorithm: the tiled back-end needs L %% %d == 0 (L = %d)", sw::TILE_W, c->L);
+        return fail(SW_ERR_UNSUPPORTED, "sw_set_algorithm: the tiled back-end needs L %% %d == 0 (L = %d)", sw::TW, c->L);
     if (algo != SW_ALGO_GENERIC && algo != SW_ALGO_TILED) return fail(SW_ERR_ARG, "sw_set_algorithm: unknown back-end %d", algo);
     c->algo = algo;
     return SW_OK;

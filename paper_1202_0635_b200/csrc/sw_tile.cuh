@@ -1,0 +1,514 @@
+// Tiled back-end (SW_ALGO_TILED), L % 128 == 0.  One sweep = three kernels:
+//
+//   K1 k_tile_label   S1 + S2a.  One CTA owns a 128 x 64 tile.
+//        phase A  bonds: Philox in registers (one call per two sites), compared with the integer threshold;
+//                 the 2 bits per site are packed into row bit masks H (bond to +x) and V (bond to +y) in
+//                 shared memory.  Bonds never go to HBM; only the bits that cross a tile edge are exported.
+//        phase B  labeling on the masks, one thread per 32-site word.  A node = a horizontal run clipped to its
+//                 word, named by the tile-local index of its first site, so all +x bonds inside a word are
+//                 merged by bit arithmetic alone.  Every node with a bond to the row above inherits (plain
+//                 store) the node above its lowest such bond; only the remaining, non-redundant up-bonds and
+//                 the bonds between words go through the shared-memory union-find (atomicMin, root = smallest
+//                 index: the "proper label ... smallest" of PAPER.md:47 at tile level).
+//        output   one uint16 per site: the tile-local index of the tile-local root, bit 15 = the cluster may
+//                 continue in another tile ("open").  Open roots also initialise their entry of the global
+//                 parent array.
+//   K2 k_seam_merge   S2b: union (global atomicMin union-find on `parent`, indexed by site) across every active
+//                     tile-crossing bond.  Touches tile-edge sites and open roots only.
+//   K3 k_tile_flip    S3 + S4.  Per tile: compact the tile-local roots, resolve the open ones to their global
+//                     root (short chase), draw the cluster decision from the CLUSTER stream keyed on that root
+//                     -- once per root, not once per site (the paper draws one per label number) --
+//                     then every site looks its root's decision up in shared memory and updates its spin.
+//
+// The root of a cluster is its minimum site index at both levels (row-major order inside a tile equals the
+// order of the global indices), so spins, labels and observables equal the oracle's bit for bit.
+// HBM traffic per site and sweep: K1 1 B (spins) + 2 B (labels); K3 2 B (labels) [+ 1 B spins, clock] + 1 B.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "sw_generic.cuh"
+#include "sw_philox.cuh"
+
+namespace sw {
+
+constexpr int TW = 128;                 // sites per tile row = 4 words of 32
+constexpr int TH = 64;                  // rows per tile
+constexpr int NWORD = TW / 32;
+constexpr int TILE_SITES = TW * TH;     // 8192 -> 13-bit local index
+constexpr int TILE_THREADS = TH * NWORD;  // one thread per word (256)
+constexpr int ROWS_PER_WARP = 8;        // TILE_THREADS / 32 warps x 8 rows = TH
+constexpr uint32_t LMASK = 0x3FFFu;     // local index field of a label
+constexpr uint32_t LOPEN = 0x8000u;     // cluster may continue in another tile
+static_assert(TILE_SITES <= (int)LMASK + 1, "local index must fit the label field");
+static_assert((TILE_THREADS / 32) * ROWS_PER_WARP == TH, "phase A row split");
+
+struct TiledState {
+    uint16_t *lab16 = nullptr;   // [L][L] tile-local root of every site (+ LOPEN)
+    uint32_t *hedge = nullptr;   // [L/128][L/32]  bit (y & 31) of word y >> 5: +x bond of column 128 tx + 127, row y
+    uint32_t *vedge = nullptr;   // [L/TH][L/32]   bit (x & 31) of word x >> 5: +y bond of row TH ty + TH - 1, column x
+    int L = 0;
+};
+
+static inline bool tiled_supported(int L) { return L >= TW && L % TW == 0 && L % TH == 0; }
+
+static inline size_t tiled_workspace_bytes(int L)
+{
+    if (!tiled_supported(L)) return 0;
+    const size_t N = (size_t)L * L;
+    return 2 * N + 1024 + (size_t)(L / TW) * (L / 32) * 4 + 1024 + (size_t)(L / TH) * (L / 32) * 4 + 1024;
+}
+
+// ---- shared-memory union-find by minimum index (same scheme as uf_union in sw_generic.cuh) ------------------
+__device__ __forceinline__ uint32_t sfind_halve(volatile uint32_t *lab, uint32_t a)
+{
+    uint32_t cur = lab[a];
+    if (cur != a) {
+        uint32_t prev = a, next;
+        while (cur > (next = lab[cur])) {
+            lab[prev] = next;
+            prev = cur;
+            cur = next;
+        }
+    }
+    return cur;
+}
+
+__device__ __forceinline__ void sunion(uint32_t *lab, uint32_t a, uint32_t b)
+{
+    for (;;) {
+        a = sfind_halve(lab, a);
+        b = sfind_halve(lab, b);
+        if (a == b) return;
+        if (a < b) { const uint32_t tmp = a; a = b; b = tmp; }
+        const uint32_t old = atomicMin(lab + a, b);   // a > b
+        if (old == a) return;
+        a = old;
+    }
+}
+
+// first site (bit position) of the segment that holds bit k; S = mask of segment starts (bit 0 always set)
+__device__ __forceinline__ uint32_t seg_start(uint32_t S, uint32_t k) { return 31u - __clz(S & ((2u << k) - 1u)); }
+
+// K1.  grid = tiles, block = TILE_THREADS.  MODEL 0 = Potts, 1 = clock.
+template <int MODEL>
+__global__ void __launch_bounds__(TILE_THREADS)
+k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ spins, uint16_t *__restrict__ lab16,
+             int32_t *__restrict__ parent, uint32_t *__restrict__ hedge, uint32_t *__restrict__ vedge)
+{
+    __shared__ uint32_t s_H[TH][NWORD];
+    __shared__ uint32_t s_V[TH][NWORD];
+    __shared__ uint32_t s_lab[TILE_SITES];
+    __shared__ uint32_t s_table[MODEL == 1 ? (2 * 16) * (2 * 16) : 1];
+
+    const uint32_t L = (uint32_t)md.L;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t tiles_x = L / TW;
+    const uint32_t tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
+    const uint32_t x0 = tx * TW, y0 = ty * TH;
+    const uint32_t q2 = 2u * (uint32_t)md.q;
+    uint32_t m = 0u;
+    if (MODEL == 1) {
+        for (uint32_t k = tid; k < q2 * q2; k += TILE_THREADS) s_table[k] = md.table[k];
+        m = axis_of_sweep(key, t, (uint32_t)md.q);
+        __syncthreads();
+    }
+
+    // ---------------- phase A: bonds of rows 8 warp .. 8 warp + 7, four sites per lane ----------------------
+    {
+        const uint32_t gx = x0 + 4u * lane;
+        const uint32_t xr = (x0 + TW == L) ? 0u : x0 + TW;   // halo column (periodic)
+        const uint32_t ly0 = warp * ROWS_PER_WARP;
+        uint32_t row[ROWS_PER_WARP + 1], hal[ROWS_PER_WARP];
+#pragma unroll
+        for (int j = 0; j <= ROWS_PER_WARP; ++j) {
+            uint32_t gy = y0 + ly0 + j;
+            if (gy == L) gy = 0u;
+            row[j] = *reinterpret_cast<const uint32_t *>(spins + (size_t)gy * L + gx);
+            if (j < ROWS_PER_WARP) hal[j] = (lane == 31u) ? (uint32_t)spins[(size_t)gy * L + xr] : 0u;
+        }
+#pragma unroll
+        for (int j = 0; j < ROWS_PER_WARP; ++j) {
+            const uint32_t cur = row[j], nxt = row[j + 1];
+            uint32_t rn = __shfl_down_sync(0xFFFFFFFFu, cur, 1) & 0xFFu;
+            if (lane == 31u) rn = hal[j];
+            const uint32_t right = (cur >> 8) | (rn << 24);       // byte k = +x neighbour of site k
+            const uint32_t i0 = (y0 + ly0 + j) * L + gx;
+            uint32_t wa[4], wb[4];
+            philox_stream<STREAM_BOND>(key, i0 >> 1, t, wa);
+            philox_stream<STREAM_BOND>(key, (i0 >> 1) + 1u, t, wb);
+            uint32_t hn = 0u, vn = 0u;
+            if (MODEL == 0) {
+                const uint32_t th = md.thr_potts;
+                const uint32_t dx = cur ^ right, dy = cur ^ nxt;   // byte k zero <=> equal spins
+                hn |= (wa[0] < th && (dx & 0x000000FFu) == 0u) ? 1u : 0u;
+                hn |= (wa[2] < th && (dx & 0x0000FF00u) == 0u) ? 2u : 0u;
+                hn |= (wb[0] < th && (dx & 0x00FF0000u) == 0u) ? 4u : 0u;
+                hn |= (wb[2] < th && (dx & 0xFF000000u) == 0u) ? 8u : 0u;
+                vn |= (wa[1] < th && (dy & 0x000000FFu) == 0u) ? 1u : 0u;
+                vn |= (wa[3] < th && (dy & 0x0000FF00u) == 0u) ? 2u : 0u;
+                vn |= (wb[1] < th && (dy & 0x00FF0000u) == 0u) ? 4u : 0u;
+                vn |= (wb[3] < th && (dy & 0xFF000000u) == 0u) ? 8u : 0u;
+            } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t c = clock_c((cur >> (8 * k)) & 0xFFu, m, q2);
+                    const uint32_t cr = clock_c((right >> (8 * k)) & 0xFFu, m, q2);
+                    const uint32_t cd = clock_c((nxt >> (8 * k)) & 0xFFu, m, q2);
+                    const uint32_t wh = (k < 2) ? wa[2 * k] : wb[2 * (k - 2)];
+                    const uint32_t wv = (k < 2) ? wa[2 * k + 1] : wb[2 * (k - 2) + 1];
+                    hn |= (wh < s_table[c * q2 + cr]) ? (1u << k) : 0u;
+                    vn |= (wv < s_table[c * q2 + cd]) ? (1u << k) : 0u;
+                }
+            }
+            // gather the nibbles of 8 lanes into one 32-site word: H in the low half, V in the high half
+            uint32_t c = hn | (vn << 16);
+            c |= __shfl_down_sync(0xFFFFFFFFu, c, 1) << 4;
+            c |= __shfl_down_sync(0xFFFFFFFFu, c, 2) << 8;
+            const uint32_t c4 = __shfl_down_sync(0xFFFFFFFFu, c, 4);
+            if ((lane & 7u) == 0u) {
+                s_H[ly0 + j][lane >> 3] = (c & 0xFFFFu) | (c4 << 16);
+                s_V[ly0 + j][lane >> 3] = (c >> 16) | (c4 & 0xFFFF0000u);
+            }
+        }
+    }
+    __syncthreads();
+
+    // bonds that leave the tile: exported for K2, never used by the tile-local graph below
+    if (tid < (uint32_t)TH) {
+        const uint32_t b = __ballot_sync(0xFFFFFFFFu, (s_H[tid][NWORD - 1] >> 31) & 1u);
+        if (lane == 0u) hedge[(size_t)tx * (L / 32) + (y0 >> 5) + warp] = b;
+    }
+    if (tid < (uint32_t)NWORD) vedge[(size_t)ty * (L / 32) + (x0 >> 5) + tid] = s_V[TH - 1][tid];
+
+    // ---------------- phase B: one thread per word --------------------------------------------------------
+    const uint32_t wy = tid / NWORD, ww = tid % NWORD;
+    const uint32_t base = wy * TW + ww * 32u;                 // local index of the word's first site
+    const uint32_t h = s_H[wy][ww];
+    const uint32_t hin = h & 0x7FFFFFFFu;                     // bonds inside the word
+    const uint32_t S = ~(hin << 1);                           // segment starts
+    uint32_t u = 0u, ha = 0u;                                 // bonds to the row above / its in-word bonds
+    if (wy > 0u) { u = s_V[wy - 1][ww]; ha = s_H[wy - 1][ww] & 0x7FFFFFFFu; }
+    const uint32_t Sa = ~(ha << 1);
+
+    // B1: every node inherits the node above its lowest up-bond, or is its own root
+    uint32_t first = 0u;
+    {
+        uint32_t rem = S;
+        while (rem) {
+            const uint32_t s = (uint32_t)__ffs((int)rem) - 1u;
+            rem &= rem - 1u;
+            const uint32_t below_ns = rem ? ((rem & (0u - rem)) - 1u) : 0xFFFFFFFFu;
+            const uint32_t ups = u & below_ns & (0xFFFFFFFFu << s);
+            uint32_t tgt = base + s;
+            if (ups) {
+                const uint32_t f = (uint32_t)__ffs((int)ups) - 1u;
+                tgt = base - TW + seg_start(Sa, f);
+                first |= ups & (0u - ups);
+            }
+            s_lab[base + s] = tgt;
+        }
+    }
+    __syncthreads();
+
+    // B2: the other up-bonds (unless the bond to their left joins the same two nodes) and the bonds between words
+    {
+        uint32_t X = u & ~first & ~((u & ha & hin) << 1);
+        while (X) {
+            const uint32_t k = (uint32_t)__ffs((int)X) - 1u;
+            X &= X - 1u;
+            sunion(s_lab, base + seg_start(S, k), base - TW + seg_start(Sa, k));
+        }
+        if (ww + 1u < (uint32_t)NWORD && (h >> 31)) sunion(s_lab, base + seg_start(S, 31u), base + 32u);
+    }
+    __syncthreads();
+
+    // B3: clusters that may continue in another tile: every cluster with a site in the top row or the left column
+    // (their bonds belong to the neighbouring tiles), or with an active bond across the right or bottom edge
+    {
+        uint32_t M = 0u;
+        if (wy == 0u) M = 0xFFFFFFFFu;
+        if (ww == 0u) M |= 1u;
+        if (ww + 1u == (uint32_t)NWORD) M |= h & 0x80000000u;
+        if (wy + 1u == (uint32_t)TH) M |= s_V[wy][ww];
+        volatile uint32_t *vl = s_lab;
+        while (M) {
+            const uint32_t k = (uint32_t)__ffs((int)M) - 1u;
+            const uint32_t above = S & ~((2u << k) - 1u);          // starts after k
+            M &= above ? (0xFFFFFFFFu << ((uint32_t)__ffs((int)above) - 1u)) : 0u;   // drop the rest of this segment
+            uint32_t a = base + seg_start(S, k), p;
+            while ((p = vl[a] & LMASK) != a) a = p;
+            vl[a] = a | LOPEN;
+        }
+    }
+    __syncthreads();
+
+    // B4: flatten every node (root index + LOPEN); open roots enter the global union-find as their own parent
+    {
+        volatile uint32_t *vl = s_lab;
+        uint32_t rem = S;
+        while (rem) {
+            const uint32_t s = (uint32_t)__ffs((int)rem) - 1u;
+            rem &= rem - 1u;
+            uint32_t a = base + s, x;
+            while (((x = vl[a]) & LMASK) != a) a = x & LMASK;
+            vl[base + s] = x;
+            if (a == base + s && (x & LOPEN)) {
+                const uint32_t g = (y0 + wy) * L + x0 + ww * 32u + s;
+                parent[g] = (int32_t)g;
+            }
+        }
+    }
+    __syncthreads();
+
+    // B5: per-site labels, 8 sites (16 bytes) per thread and pass
+#pragma unroll
+    for (int c = 0; c < TILE_SITES / 8 / TILE_THREADS; ++c) {
+        const uint32_t p8 = ((uint32_t)c * TILE_THREADS + tid) * 8u;
+        const uint32_t y = p8 / TW, x = p8 % TW, w = x >> 5, k0 = x & 31u;
+        const uint32_t Sw = ~((s_H[y][w] & 0x7FFFFFFFu) << 1);
+        const uint32_t wbase = y * TW + w * 32u;
+        uint32_t v[8];
+        v[0] = s_lab[wbase + seg_start(Sw, k0)];
+#pragma unroll
+        for (int j = 1; j < 8; ++j) v[j] = ((Sw >> (k0 + j)) & 1u) ? s_lab[wbase + k0 + j] : v[j - 1];
+        uint4 o;
+        o.x = v[0] | (v[1] << 16); o.y = v[2] | (v[3] << 16); o.z = v[4] | (v[5] << 16); o.w = v[6] | (v[7] << 16);
+        *reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + y) * L + x0 + x) = o;
+    }
+}
+
+// Global site index of the tile-local root named by label word `v` of a site of the tile with origin (X0, Y0).
+__device__ __forceinline__ uint32_t root_site(uint32_t v, uint32_t X0, uint32_t Y0, uint32_t L)
+{
+    const uint32_t p = v & LMASK;
+    return (Y0 + p / TW) * L + X0 + p % TW;
+}
+
+__device__ __forceinline__ uint32_t root_site_of(const uint16_t *__restrict__ lab16, uint32_t x, uint32_t y, uint32_t L)
+{
+    return root_site(lab16[(size_t)y * L + x], x - x % TW, y - y % TH, L);
+}
+
+// Tile-crossing bond e -> (active, tile-local roots a and b of its two ends, as global site indices).
+// First the (L/128)*L right-edge bonds, then the (L/TH)*L bottom-edge bonds.
+__device__ __forceinline__ bool seam_bond(uint32_t e, uint32_t L, const uint32_t *__restrict__ hedge,
+                                          const uint32_t *__restrict__ vedge, const uint16_t *__restrict__ lab16,
+                                          uint32_t &a, uint32_t &b)
+{
+    const uint32_t nh = (L / TW) * L;
+    if (e < nh) {
+        const uint32_t tx = e / L, y = e - tx * L;
+        if (!((hedge[tx * (L / 32) + (y >> 5)] >> (y & 31u)) & 1u)) return false;
+        const uint32_t x = tx * TW + TW - 1u;
+        const uint32_t xr = (x + 1u == L) ? 0u : x + 1u;
+        a = root_site_of(lab16, x, y, L);
+        b = root_site_of(lab16, xr, y, L);
+        return true;
+    }
+    const uint32_t f = e - nh;
+    const uint32_t ty = f / L, x = f - ty * L;
+    if (!((vedge[ty * (L / 32) + (x >> 5)] >> (x & 31u)) & 1u)) return false;
+    const uint32_t y = ty * TH + TH - 1u;
+    const uint32_t yd = (y + 1u == L) ? 0u : y + 1u;
+    a = root_site_of(lab16, x, y, L);
+    b = root_site_of(lab16, x, yd, L);
+    return true;
+}
+
+// K2.  One thread per tile-edge bond position.
+__global__ void __launch_bounds__(256)
+k_seam_merge(Model md, const uint32_t *__restrict__ hedge, const uint32_t *__restrict__ vedge,
+             const uint16_t *__restrict__ lab16, int32_t *parent, unsigned long long *stats)
+{
+    const uint32_t L = (uint32_t)md.L;
+    const uint32_t ne = (L / TW) * L + (L / TH) * L;
+    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t a = 0xFFFFFFFFu, b = 0xFFFFFFFFu;
+    const bool act = (e < ne) && seam_bond(e, L, hedge, vedge, lab16, a, b);
+    // the neighbouring edge position often joins the same pair of tile-local clusters: skip the repeat
+    const uint32_t pa = __shfl_up_sync(0xFFFFFFFFu, a, 1), pb = __shfl_up_sync(0xFFFFFFFFu, b, 1);
+    const bool dup = (threadIdx.x & 31u) != 0u && pa == a && pb == b;
+    if (act && !dup) {
+        if (stats) atomicAdd(stats + 1, 1ull);
+        uf_union(parent, (int32_t)a, (int32_t)b);
+    }
+}
+
+// K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).
+template <int MODEL>
+__global__ void __launch_bounds__(TILE_THREADS)
+k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ lab16, const int32_t *__restrict__ parent,
+            uint8_t *__restrict__ spins)
+{
+    constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
+    __shared__ uint16_t s_roots[TILE_SITES];   // compacted tile-local roots (+ LOPEN)
+    __shared__ uint8_t s_dec[TILE_SITES];      // decision of the cluster whose tile-local root is p
+    __shared__ uint32_t s_count;
+
+    const uint32_t L = (uint32_t)md.L;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u;
+    const uint32_t tiles_x = L / TW;
+    const uint32_t tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
+    const uint32_t x0 = tx * TW, y0 = ty * TH;
+    if (tid == 0u) s_count = 0u;
+
+    uint4 lab[PASSES];
+    uint32_t rootm = 0u, openm = 0u;   // bit 8c + j: site j of pass c is a tile-local root / an open one
+#pragma unroll
+    for (int c = 0; c < PASSES; ++c) {
+        const uint32_t p8 = ((uint32_t)c * TILE_THREADS + tid) * 8u;
+        lab[c] = *reinterpret_cast<const uint4 *>(lab16 + (size_t)(y0 + p8 / TW) * L + x0 + p8 % TW);
+        const uint32_t w[4] = { lab[c].x, lab[c].y, lab[c].z, lab[c].w };
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const uint32_t v = (w[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
+            if ((v & LMASK) == p8 + j) {
+                rootm |= 1u << (8 * c + j);
+                if (v & LOPEN) openm |= 1u << (8 * c + j);
+            }
+        }
+    }
+    __syncthreads();   // s_count = 0 visible
+
+    // compact the roots of the tile: warp prefix sum of the per-thread counts, one atomic per warp
+    {
+        const uint32_t n = __popc(rootm);
+        uint32_t incl = n;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+            if (lane >= (uint32_t)d) incl += o;
+        }
+        uint32_t wbase = 0u;
+        if (lane == 31u) wbase = atomicAdd(&s_count, incl);
+        wbase = __shfl_sync(0xFFFFFFFFu, wbase, 31);
+        uint32_t at = wbase + incl - n, rm = rootm;
+        while (rm) {
+            const uint32_t k = (uint32_t)__ffs((int)rm) - 1u;
+            rm &= rm - 1u;
+            const uint32_t p = (((k >> 3) * TILE_THREADS + tid) * 8u) + (k & 7u);
+            s_roots[at++] = (uint16_t)(p | (((openm >> k) & 1u) ? LOPEN : 0u));
+        }
+    }
+    __syncthreads();
+
+    // one decision per root: open roots chase to the global root first (S3; R5 CLUSTER stream)
+    const uint32_t nroots = s_count;
+    for (uint32_t i = tid; i < nroots; i += TILE_THREADS) {
+        const uint32_t e = s_roots[i];
+        const uint32_t p = e & LMASK;
+        uint32_t r = (y0 + p / TW) * L + x0 + p % TW;
+        if (e & LOPEN) {
+            int32_t a = (int32_t)r, pa;
+            while ((pa = __ldg(parent + a)) != a) a = pa;
+            r = (uint32_t)a;
+        }
+        uint32_t w[4];
+        philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
+        const uint32_t ww = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
+        s_dec[p] = (uint8_t)(MODEL == 0 ? mulhi_q(ww, (uint32_t)md.q) : (ww >> 31));
+    }
+    __syncthreads();
+
+    // S4: every site takes the decision of its root
+    uint32_t m = 0u;
+    if (MODEL == 1) m = axis_of_sweep(key, t, (uint32_t)md.q);
+#pragma unroll
+    for (int c = 0; c < PASSES; ++c) {
+        const uint32_t p8 = ((uint32_t)c * TILE_THREADS + tid) * 8u;
+        uint8_t *dst = spins + (size_t)(y0 + p8 / TW) * L + x0 + p8 % TW;
+        const uint32_t w[4] = { lab[c].x, lab[c].y, lab[c].z, lab[c].w };
+        uint32_t d[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) d[j] = s_dec[(w[j >> 1] >> (16 * (j & 1))) & LMASK];
+        uint2 o;
+        if (MODEL == 0) {
+            o.x = d[0] | (d[1] << 8) | (d[2] << 16) | (d[3] << 24);
+            o.y = d[4] | (d[5] << 8) | (d[6] << 16) | (d[7] << 24);
+        } else {
+            const uint2 old = *reinterpret_cast<const uint2 *>(dst);
+            const uint32_t q = (uint32_t)md.q;
+            uint32_t s[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                s[j] = (((j < 4) ? old.x : old.y) >> (8 * (j & 3))) & 0xFFu;
+                if (d[j]) {
+                    const uint32_t vv = m + q - s[j];          // in (0, 2q)
+                    s[j] = vv >= q ? vv - q : vv;
+                }
+            }
+            o.x = s[0] | (s[1] << 8) | (s[2] << 16) | (s[3] << 24);
+            o.y = s[4] | (s[5] << 8) | (s[6] << 16) | (s[7] << 24);
+        }
+        *reinterpret_cast<uint2 *>(dst) = o;
+    }
+}
+
+// Debug export (sw_get_labels): canonical root of every site.
+__global__ void k_resolve_labels(Model md, const uint16_t *__restrict__ lab16, const int32_t *__restrict__ parent,
+                                 int32_t *__restrict__ out)
+{
+    const uint32_t L = (uint32_t)md.L;
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= md.N) return;
+    const uint32_t y = i / L, x = i - y * L;
+    const uint32_t v = lab16[i];
+    int32_t a = (int32_t)root_site(v, x - x % TW, y - y % TH, L);
+    if (v & LOPEN) a = uf_find(parent, a);
+    out[i] = a;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------
+static inline int tiled_init(TiledState &st, const Model &md, char *ws)
+{
+    const size_t L = (size_t)md.L;
+    st.L = md.L;
+    size_t off = 0;
+    st.lab16 = reinterpret_cast<uint16_t *>(ws);
+    off += (2 * L * L + 1023) / 1024 * 1024;
+    st.hedge = reinterpret_cast<uint32_t *>(ws + off);
+    off += ((L / TW) * (L / 32) * 4 + 1023) / 1024 * 1024;
+    st.vedge = reinterpret_cast<uint32_t *>(ws + off);
+    return 0;
+}
+
+constexpr int TILED_NUM_KERNELS = 3;
+static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k_seam_merge", "k_tile_flip" };
+
+// ev (optional): ev[0] is recorded before the first kernel, ev[k+1] after kernel k.
+static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, uint8_t *spins,
+                              int32_t *parent, cudaStream_t stream, unsigned long long *stats, uint64_t *launches,
+                              cudaEvent_t *ev)
+{
+    const uint32_t L = (uint32_t)md.L;
+    const uint32_t tiles = (L / TW) * (L / TH);
+    const uint32_t ne = (L / TW) * L + (L / TH) * L;
+    if (ev) cudaEventRecord(ev[0], stream);
+    if (md.model == 0)
+        k_tile_label<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, spins, st.lab16, parent, st.hedge, st.vedge);
+    else
+        k_tile_label<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, spins, st.lab16, parent, st.hedge, st.vedge);
+    if (ev) cudaEventRecord(ev[1], stream);
+    k_seam_merge<<<(ne + 255) / 256, 256, 0, stream>>>(md, st.hedge, st.vedge, st.lab16, parent, stats);
+    if (ev) cudaEventRecord(ev[2], stream);
+    if (md.model == 0)
+        k_tile_flip<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, st.lab16, parent, spins);
+    else
+        k_tile_flip<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, st.lab16, parent, spins);
+    if (ev) cudaEventRecord(ev[3], stream);
+    *launches += 3;
+    return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
+}
+
+static inline int tiled_resolve_labels(TiledState &st, const Model &md, const int32_t *parent, int32_t *out,
+                                       cudaStream_t stream, uint64_t *launches)
+{
+    k_resolve_labels<<<(md.N + 255) / 256, 256, 0, stream>>>(md, st.lab16, parent, out);
+    *launches += 1;
+    return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
+}
+
+}  // namespace sw
