@@ -106,11 +106,13 @@ int sw_set_algorithm(sw_ctx *ctx, int algo);
 int sw_get_algorithm(sw_ctx *ctx); /* the back-end actually in use (never SW_ALGO_AUTO) */
 
 /* Labeling work counters accumulated since creation (the analogue of the paper's iteration counts,
- * PAPER.md:75): out[0] = sweeps counted, out[1] = cross-tile merge attempts, out[2] = merge atomics
- * that changed a root, out[3] = open tile roots processed by the flatten pass.  HOST output of 4 doubles;
- * counters are only collected after sw_enable_stats(ctx, 1) (they cost atomics). */
+ * PAPER.md:75), HOST output of SW_NUM_STATS doubles: out[0] = sweeps counted, out[1] = cross-tile merge attempts,
+ * out[2] = tile-local nodes (horizontal runs), out[3] = tile-local union edges, out[4] = pointer hops of the
+ * tile-local resolve pass, out[5..7] reserved (0).  Counters are only collected after sw_enable_stats(ctx, 1)
+ * (they cost atomics). */
+#define SW_NUM_STATS 8
 int sw_enable_stats(sw_ctx *ctx, int on);
-int sw_stats(sw_ctx *ctx, double *out4);
+int sw_stats(sw_ctx *ctx, double *out);
 
 /* n sweeps with every kernel bracketed by CUDA events on the context's stream (one stream sync per sweep, so
  * this is a measurement mode, not the production path): ms_out[k] (HOST, SW_MAX_KERNELS doubles) receives the

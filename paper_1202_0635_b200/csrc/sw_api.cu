@@ -449,10 +449,10 @@ int sw_enable_stats(sw_ctx *c, int on)
 int sw_stats(sw_ctx *c, double *out4)
 {
     if (!c || !out4) return fail(SW_ERR_ARG, "sw_stats: NULL argument");
-    unsigned long long h[4];
+    unsigned long long h[8];
     CU_TRY(cudaMemcpyAsync(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CU_TRY(cudaStreamSynchronize(c->stream));
-    for (int k = 0; k < 4; ++k) out4[k] = (double)h[k];
+    for (int k = 0; k < 8; ++k) out4[k] = (double)h[k];
     out4[0] = (double)c->stat_sweeps;
     return SW_OK;
 }

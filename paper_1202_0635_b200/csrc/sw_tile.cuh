@@ -40,7 +40,9 @@ constexpr int TILE_THREADS = TH * NWORD;  // one thread per word (256)
 constexpr int ROWS_PER_WARP = 8;        // TILE_THREADS / 32 warps x 8 rows = TH
 constexpr uint32_t LMASK = 0x3FFFu;     // local index field of a label
 constexpr uint32_t LOPEN = 0x8000u;     // cluster may continue in another tile
-static_assert(TILE_SITES <= (int)LMASK + 1, "local index must fit the label field");
+constexpr int LAB_WORDS = TILE_SITES + TILE_SITES / 32;   // skewed tile-local index sp = p + (p >> 5)
+constexpr int EDGE_CAP = 256;           // union edges listed per warp (more are handled by their own thread)
+static_assert(LAB_WORDS <= (int)LMASK + 1, "skewed local index must fit the label field");
 static_assert((TILE_THREADS / 32) * ROWS_PER_WARP == TH, "phase A row split");
 
 struct TiledState {
@@ -91,14 +93,19 @@ __device__ __forceinline__ void sunion(uint32_t *lab, uint32_t a, uint32_t b)
 __device__ __forceinline__ uint32_t seg_start(uint32_t S, uint32_t k) { return 31u - __clz(S & ((2u << k) - 1u)); }
 
 // K1.  grid = tiles, block = TILE_THREADS.  MODEL 0 = Potts, 1 = clock.
+#ifndef SW_LABEL_MINB
+#define SW_LABEL_MINB 5
+#endif
 template <int MODEL>
-__global__ void __launch_bounds__(TILE_THREADS)
+__global__ void __launch_bounds__(TILE_THREADS, SW_LABEL_MINB)
 k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ spins, uint16_t *__restrict__ lab16,
-             int32_t *__restrict__ parent, uint32_t *__restrict__ hedge, uint32_t *__restrict__ vedge)
+             int32_t *__restrict__ parent, uint32_t *__restrict__ hedge, uint32_t *__restrict__ vedge,
+             unsigned long long *stats)
 {
     __shared__ uint32_t s_H[TH][NWORD];
     __shared__ uint32_t s_V[TH][NWORD];
-    __shared__ uint32_t s_lab[TILE_SITES];
+    __shared__ uint32_t s_lab[LAB_WORDS];
+    __shared__ uint32_t s_edge[TILE_THREADS / 32][EDGE_CAP + 1];   // + dump slot
     __shared__ uint32_t s_table[MODEL == 1 ? (2 * 16) * (2 * 16) : 1];
 
     const uint32_t L = (uint32_t)md.L;
@@ -182,106 +189,215 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     if (tid < (uint32_t)NWORD) vedge[(size_t)ty * (L / 32) + (x0 >> 5) + tid] = s_V[TH - 1][tid];
 
     // ---------------- phase B: one thread per word --------------------------------------------------------
+    // All label values are SKEWED tile-local indices sp = p + (p >> 5) (one pad word per 32-site word), so that the
+    // 32 lanes of a warp, which own 32 different words, hit 32 different banks when they touch the same bit position.
     const uint32_t wy = tid / NWORD, ww = tid % NWORD;
-    const uint32_t base = wy * TW + ww * 32u;                 // local index of the word's first site
+    const uint32_t sb = 33u * tid;                            // skewed index of the word's first site
+    const uint32_t sbu = sb - 132u;                           // ... of the word above (tid - 4)
     const uint32_t h = s_H[wy][ww];
     const uint32_t hin = h & 0x7FFFFFFFu;                     // bonds inside the word
-    const uint32_t S = ~(hin << 1);                           // segment starts
+    const uint32_t S = ~(hin << 1);                           // run starts (bit 0 always)
+    const uint32_t E = ~hin;                                  // run ends (bit 31 always)
     uint32_t u = 0u, ha = 0u;                                 // bonds to the row above / its in-word bonds
     if (wy > 0u) { u = s_V[wy - 1][ww]; ha = s_H[wy - 1][ww] & 0x7FFFFFFFu; }
     const uint32_t Sa = ~(ha << 1);
-
-    // B1: every node inherits the node above its lowest up-bond, or is its own root
-    uint32_t first = 0u;
+    // lowest up-bond of every run, by carry propagation: adding the up-bonds that have a right neighbour in their
+    // run (g) to the link mask ripples a carry to the end of the run, where the link bit is 0 and absorbs it.
+    const uint32_t g = u & hin, sum = hin + g;
+    const uint32_t first = (g & (sum ^ hin)) | (u & ~hin & ~sum);
+    // up-bonds that still need a union: not the first of their run, and not parallel to the bond on their left
+    const uint32_t X = u & ~first & ~((u & ha & hin) << 1);
+    const bool hedge_out = (ww + 1u < (uint32_t)NWORD) && (h >> 31);
+    uint32_t epos;                                            // this thread's first slot in the warp's edge list
+    uint32_t etotal;
     {
-        uint32_t rem = S;
-        while (rem) {
-            const uint32_t s = (uint32_t)__ffs((int)rem) - 1u;
-            rem &= rem - 1u;
-            const uint32_t below_ns = rem ? ((rem & (0u - rem)) - 1u) : 0xFFFFFFFFu;
-            const uint32_t ups = u & below_ns & (0xFFFFFFFFu << s);
-            uint32_t tgt = base + s;
-            if (ups) {
-                const uint32_t f = (uint32_t)__ffs((int)ups) - 1u;
-                tgt = base - TW + seg_start(Sa, f);
-                first |= ups & (0u - ups);
+        const uint32_t n = __popc(X) + (hedge_out ? 1u : 0u);
+        uint32_t incl = n;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+            if (lane >= (uint32_t)d) incl += o;
+        }
+        etotal = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        epos = incl - n;
+    }
+    const uint32_t epos0 = epos;
+
+    // B1: one left-to-right pass over the 32 bit positions (straight-line, no bit searches).  Every run inherits the
+    // run above its lowest up-bond (plain store) or becomes its own root; the other up-bonds go to the edge list.
+    uint32_t rs = 0u;                                         // start of the current run
+    {
+        uint32_t as = 0u, tgt = 132u;                         // start of the run above; target relative to sbu
+        uint32_t *el = s_edge[warp];
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            const uint32_t bit = 1u << k;
+            if (Sa & bit) as = (uint32_t)k;
+            if (S & bit) { rs = (uint32_t)k; tgt = 132u + (uint32_t)k; }
+            if (first & bit) tgt = as;
+            {   // listed edge, or a store to the dump slot EDGE_CAP (branch-free)
+                const uint32_t isx = (X >> k) & 1u;
+                uint32_t slot = isx ? epos : (uint32_t)EDGE_CAP;
+                slot = slot < (uint32_t)EDGE_CAP ? slot : (uint32_t)EDGE_CAP;
+                el[slot] = (sb + rs) | ((sbu + as) << 16);
+                epos += isx;
             }
-            s_lab[base + s] = tgt;
+            if (E & bit) s_lab[sb + rs] = sbu + tgt;
+        }
+        if (hedge_out) {                                      // bond to the next word of the row
+            if (epos < (uint32_t)EDGE_CAP) el[epos] = (sb + 33u) | ((sb + rs) << 16);
+            ++epos;
         }
     }
     __syncthreads();
+#ifndef SW_JUMP_ROUNDS
+#define SW_JUMP_ROUNDS 0
+#endif
+#ifndef SW_B4_WRITEBACK
+#define SW_B4_WRITEBACK 1
+#endif
+    // B1b: pointer jumping on the inheritance forest (straight-line, all loads of a round independent)
+#pragma unroll 1
+    for (int r = 0; r < SW_JUMP_ROUNDS; ++r) {
+        uint32_t pp[32];
+#pragma unroll
+        for (int k = 0; k < 32; ++k) pp[k] = ((S >> k) & 1u) ? s_lab[sb + k] : 0u;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) if ((S >> k) & 1u) pp[k] = s_lab[pp[k]];
+#pragma unroll
+        for (int k = 0; k < 32; ++k) if ((S >> k) & 1u) s_lab[sb + k] = pp[k];
+        __syncthreads();
+    }
 
-    // B2: the other up-bonds (unless the bond to their left joins the same two nodes) and the bonds between words
+    // B2: the warp's edges, one per lane and round (union-find by minimum index: PAPER.md:47 at tile level)
     {
-        uint32_t X = u & ~first & ~((u & ha & hin) << 1);
-        while (X) {
-            const uint32_t k = (uint32_t)__ffs((int)X) - 1u;
-            X &= X - 1u;
-            sunion(s_lab, base + seg_start(S, k), base - TW + seg_start(Sa, k));
+        const uint32_t ne = etotal < (uint32_t)EDGE_CAP ? etotal : (uint32_t)EDGE_CAP;
+        // Every lane walks its own edges at its own pace (one pointer hop of both ends per trip), so a long
+        // chain in one lane does not stall the other lanes edge by edge.
+        uint32_t e = lane;
+        if (e < ne) {
+            volatile uint32_t *vl = s_lab;
+            uint32_t v = s_edge[warp][e];
+            uint32_t a0 = v & 0xFFFFu, b0 = v >> 16, a = a0, b = b0;
+            for (;;) {
+                const uint32_t pa = vl[a], pb = vl[b];
+                if (pa != a || pb != b) { a = pa; b = pb; continue; }
+                uint32_t lo = a;
+                if (a != b) {
+                    const uint32_t hi = a > b ? a : b;
+                    lo = a > b ? b : a;
+                    const uint32_t old = atomicMin(s_lab + hi, lo);
+                    if (old != hi) { a = old; b = lo; continue; }   // hi had a parent already: keep it connected to lo
+                }
+                if (vl[a0] > lo && a0 != lo) vl[a0] = lo;           // both ends straight to the root (an ancestor)
+                if (vl[b0] > lo && b0 != lo) vl[b0] = lo;
+                e += 32u;
+                if (e >= ne) break;
+                v = s_edge[warp][e];
+                a0 = v & 0xFFFFu; b0 = v >> 16; a = a0; b = b0;
+            }
         }
-        if (ww + 1u < (uint32_t)NWORD && (h >> 31)) sunion(s_lab, base + seg_start(S, 31u), base + 32u);
+        if (etotal > (uint32_t)EDGE_CAP && epos > (uint32_t)EDGE_CAP) {
+            // rare: the list overflowed; this thread unions its unlisted edges itself
+            uint32_t slot = epos0, Xr = X;
+            while (Xr) {
+                const uint32_t k = (uint32_t)__ffs((int)Xr) - 1u;
+                Xr &= Xr - 1u;
+                if (slot >= (uint32_t)EDGE_CAP) sunion(s_lab, sb + seg_start(S, k), sbu + seg_start(Sa, k));
+                ++slot;
+            }
+            if (hedge_out && slot >= (uint32_t)EDGE_CAP) sunion(s_lab, sb + 33u, sb + rs);
+        }
     }
     __syncthreads();
 
     // B3: clusters that may continue in another tile: every cluster with a site in the top row or the left column
-    // (their bonds belong to the neighbouring tiles), or with an active bond across the right or bottom edge
+    // (their bonds belong to the neighbouring tiles), or with an active bond across the right or bottom edge.
+    // One boundary site per thread and pass; only the first site of a run (or of a bonded stretch) does the work.
     {
-        uint32_t M = 0u;
-        if (wy == 0u) M = 0xFFFFFFFFu;
-        if (ww == 0u) M |= 1u;
-        if (ww + 1u == (uint32_t)NWORD) M |= h & 0x80000000u;
-        if (wy + 1u == (uint32_t)TH) M |= s_V[wy][ww];
         volatile uint32_t *vl = s_lab;
-        while (M) {
-            const uint32_t k = (uint32_t)__ffs((int)M) - 1u;
-            const uint32_t above = S & ~((2u << k) - 1u);          // starts after k
-            M &= above ? (0xFFFFFFFFu << ((uint32_t)__ffs((int)above) - 1u)) : 0u;   // drop the rest of this segment
-            uint32_t a = base + seg_start(S, k), p;
-            while ((p = vl[a] & LMASK) != a) a = p;
-            vl[a] = a | LOPEN;
+        uint32_t c0 = 0xFFFFFFFFu, c1 = 0xFFFFFFFFu;
+        if (tid < (uint32_t)TW) {
+            const uint32_t w = tid >> 5, k = tid & 31u;
+            const uint32_t S0 = ~((s_H[0][w] & 0x7FFFFFFFu) << 1);
+            if ((S0 >> k) & 1u) c0 = 33u * w + k;
+            const uint32_t hb = s_H[TH - 1][w] & 0x7FFFFFFFu, vb = s_V[TH - 1][w];
+            const bool dup = k > 0u && ((vb & hb) >> (k - 1u)) & 1u;
+            if (((vb >> k) & 1u) && !dup) c1 = 33u * ((TH - 1) * NWORD + w) + seg_start(~(hb << 1), k);
+        } else if (tid < (uint32_t)(TW + TH)) {
+            c0 = 33u * ((tid - TW) * NWORD);
+        } else if (tid < (uint32_t)(TW + 2 * TH)) {
+            const uint32_t r = tid - (TW + TH);
+            const uint32_t hr = s_H[r][NWORD - 1];
+            if (hr >> 31) c0 = 33u * (r * NWORD + NWORD - 1) + seg_start(~((hr & 0x7FFFFFFFu) << 1), 31u);
         }
-    }
-    __syncthreads();
-
-    // B4: flatten every node (root index + LOPEN); open roots enter the global union-find as their own parent
-    {
-        volatile uint32_t *vl = s_lab;
-        uint32_t rem = S;
-        while (rem) {
-            const uint32_t s = (uint32_t)__ffs((int)rem) - 1u;
-            rem &= rem - 1u;
-            uint32_t a = base + s, x;
-            while (((x = vl[a]) & LMASK) != a) a = x & LMASK;
-            vl[base + s] = x;
-            if (a == base + s && (x & LOPEN)) {
-                const uint32_t g = (y0 + wy) * L + x0 + ww * 32u + s;
-                parent[g] = (int32_t)g;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            uint32_t a = c ? c1 : c0;
+            if (a != 0xFFFFFFFFu) {
+                uint32_t p;
+                while ((p = vl[a] & LMASK) != a) a = p;
+                vl[a] = a | LOPEN;
             }
         }
     }
     __syncthreads();
 
-    // B5: per-site labels, 8 sites (16 bytes) per thread and pass
+    // B4a: resolve every run of the word to its root (+ LOPEN), lane-autonomous: one pointer hop per trip, a lane
+    // moves on to its next run as soon as one is resolved and writes the root back to the run's own entry
+    uint32_t hops = 0u;
+    {
+        volatile uint32_t *vl = s_lab;
+        uint32_t rem = S;
+        uint32_t k = 31u - (uint32_t)__clz((int)rem);        // S has bit 0 set
+        uint32_t own = sb + k, a = own;
+        for (;;) {
+            const uint32_t x = vl[a];
+            const uint32_t p = x & LMASK;
+            if (p != a) { a = p; ++hops; continue; }
+            vl[own] = x;
+            rem ^= 1u << k;
+            if (!rem) break;
+            k = 31u - (uint32_t)__clz((int)rem);
+            own = sb + k;
+            a = own;
+        }
+    }
+    __syncwarp();
+
+    // B4b: per-site labels of the word (64 contiguous bytes); open roots enter the global union-find as their
+    // own parent
+    {
+        volatile uint32_t *vl = s_lab;
+        const uint32_t g0 = (y0 + wy) * L + x0 + ww * 32u;
+        uint32_t xs[32];
 #pragma unroll
-    for (int c = 0; c < TILE_SITES / 8 / TILE_THREADS; ++c) {
-        const uint32_t p8 = ((uint32_t)c * TILE_THREADS + tid) * 8u;
-        const uint32_t y = p8 / TW, x = p8 % TW, w = x >> 5, k0 = x & 31u;
-        const uint32_t Sw = ~((s_H[y][w] & 0x7FFFFFFFu) << 1);
-        const uint32_t wbase = y * TW + w * 32u;
-        uint32_t v[8];
-        v[0] = s_lab[wbase + seg_start(Sw, k0)];
+        for (int k = 0; k < 32; ++k) xs[k] = ((S >> k) & 1u) ? vl[sb + k] : 0u;
+        uint32_t cur = 0u, o[16];
 #pragma unroll
-        for (int j = 1; j < 8; ++j) v[j] = ((Sw >> (k0 + j)) & 1u) ? s_lab[wbase + k0 + j] : v[j - 1];
-        uint4 o;
-        o.x = v[0] | (v[1] << 16); o.y = v[2] | (v[3] << 16); o.z = v[4] | (v[5] << 16); o.w = v[6] | (v[7] << 16);
-        *reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + y) * L + x0 + x) = o;
+        for (int k = 0; k < 32; ++k) {
+            if ((S >> k) & 1u) {
+                cur = xs[k];
+                if (cur == ((sb + (uint32_t)k) | LOPEN)) parent[g0 + k] = (int32_t)(g0 + k);
+            }
+            if (k & 1) o[k >> 1] |= cur << 16; else o[k >> 1] = cur;
+        }
+        uint4 *dst = reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) dst[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
+        if (stats) {
+            atomicAdd(stats + 2, (unsigned long long)__popc(S));
+            atomicAdd(stats + 3, (unsigned long long)(epos - epos0));
+            atomicAdd(stats + 4, (unsigned long long)hops);
+        }
     }
 }
 
 // Global site index of the tile-local root named by label word `v` of a site of the tile with origin (X0, Y0).
 __device__ __forceinline__ uint32_t root_site(uint32_t v, uint32_t X0, uint32_t Y0, uint32_t L)
 {
-    const uint32_t p = v & LMASK;
+    const uint32_t sp = v & LMASK;
+    const uint32_t p = sp - sp / 33u;          // undo the skew sp = p + (p >> 5)
     return (Y0 + p / TW) * L + X0 + p % TW;
 }
 
@@ -343,7 +459,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
 {
     constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
     __shared__ uint16_t s_roots[TILE_SITES];   // compacted tile-local roots (+ LOPEN)
-    __shared__ uint8_t s_dec[TILE_SITES];      // decision of the cluster whose tile-local root is p
+    __shared__ uint8_t s_dec[LAB_WORDS];       // decision of the cluster whose tile-local root is sp (skewed index)
     __shared__ uint32_t s_count;
 
     const uint32_t L = (uint32_t)md.L;
@@ -363,7 +479,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
             const uint32_t v = (w[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
-            if ((v & LMASK) == p8 + j) {
+            if ((v & LMASK) == p8 + (p8 >> 5) + j) {
                 rootm |= 1u << (8 * c + j);
                 if (v & LOPEN) openm |= 1u << (8 * c + j);
             }
@@ -387,8 +503,9 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
         while (rm) {
             const uint32_t k = (uint32_t)__ffs((int)rm) - 1u;
             rm &= rm - 1u;
-            const uint32_t p = (((k >> 3) * TILE_THREADS + tid) * 8u) + (k & 7u);
-            s_roots[at++] = (uint16_t)(p | (((openm >> k) & 1u) ? LOPEN : 0u));
+            const uint32_t p8 = ((k >> 3) * TILE_THREADS + tid) * 8u;
+            const uint32_t sp = p8 + (p8 >> 5) + (k & 7u);
+            s_roots[at++] = (uint16_t)(sp | (((openm >> k) & 1u) ? LOPEN : 0u));
         }
     }
     __syncthreads();
@@ -397,8 +514,8 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
     const uint32_t nroots = s_count;
     for (uint32_t i = tid; i < nroots; i += TILE_THREADS) {
         const uint32_t e = s_roots[i];
-        const uint32_t p = e & LMASK;
-        uint32_t r = (y0 + p / TW) * L + x0 + p % TW;
+        const uint32_t sp = e & LMASK;
+        uint32_t r = root_site(sp, x0, y0, L);
         if (e & LOPEN) {
             int32_t a = (int32_t)r, pa;
             while ((pa = __ldg(parent + a)) != a) a = pa;
@@ -407,7 +524,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
         uint32_t w[4];
         philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
         const uint32_t ww = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
-        s_dec[p] = (uint8_t)(MODEL == 0 ? mulhi_q(ww, (uint32_t)md.q) : (ww >> 31));
+        s_dec[sp] = (uint8_t)(MODEL == 0 ? mulhi_q(ww, (uint32_t)md.q) : (ww >> 31));
     }
     __syncthreads();
 
@@ -488,9 +605,9 @@ static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &
     const uint32_t ne = (L / TW) * L + (L / TH) * L;
     if (ev) cudaEventRecord(ev[0], stream);
     if (md.model == 0)
-        k_tile_label<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, spins, st.lab16, parent, st.hedge, st.vedge);
+        k_tile_label<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, spins, st.lab16, parent, st.hedge, st.vedge, stats);
     else
-        k_tile_label<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, spins, st.lab16, parent, st.hedge, st.vedge);
+        k_tile_label<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, spins, st.lab16, parent, st.hedge, st.vedge, stats);
     if (ev) cudaEventRecord(ev[1], stream);
     k_seam_merge<<<(ne + 255) / 256, 256, 0, stream>>>(md, st.hedge, st.vedge, st.lab16, parent, stats);
     if (ev) cudaEventRecord(ev[2], stream);
