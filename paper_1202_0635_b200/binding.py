@@ -208,7 +208,7 @@ class Lattice:
         _check(self._lib.sw_enable_stats(self._h, 1 if on else 0))
 
     def stats(self) -> np.ndarray:
-        out = np.zeros(8, dtype=np.float64)
+        out = np.zeros(16, dtype=np.float64)
         _check(self._lib.sw_stats(self._h, out.ctypes.data))
         return out
 

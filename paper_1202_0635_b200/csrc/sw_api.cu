@@ -63,7 +63,7 @@ Carve carve(int L, int q)
     c.table = off;  off += align_up(4 * (size_t)(2 * SW_MAX_Q) * (2 * SW_MAX_Q));
     c.obs = off;    off += align_up(8 * OBS_WORDS);
     c.flag = off;   off += align_up(64);
-    c.stats = off;  off += align_up(64);
+    c.stats = off;  off += align_up(8 * SW_NUM_STATS);
     c.ring = off;   off += align_up((size_t)REC_ROWS * OBS_WORDS * 8);
     c.tiled = off;  off += align_up(sw::tiled_workspace_bytes(L));
     c.total = off;
@@ -240,7 +240,7 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
     ok = ok && cudaMemsetAsync(c->table, 0, 4 * (size_t)(2 * SW_MAX_Q) * (2 * SW_MAX_Q), c->stream) == cudaSuccess;
     if (model == SW_CLOCK)
         ok = ok && cudaMemcpyAsync(c->table, c->thr_host.data(), 4 * c->thr_host.size(), cudaMemcpyHostToDevice, c->stream) == cudaSuccess;
-    ok = ok && cudaMemsetAsync(c->stats, 0, 64, c->stream) == cudaSuccess;
+    ok = ok && cudaMemsetAsync(c->stats, 0, 8 * SW_NUM_STATS, c->stream) == cudaSuccess;
     if (ok) {
         sw::k_init_spins<<<blocks_for((c->N + 3) / 4, 256), 256, 0, c->stream>>>(c->md, c->key, c->spins);
         c->launches += 1;
@@ -449,10 +449,10 @@ int sw_enable_stats(sw_ctx *c, int on)
 int sw_stats(sw_ctx *c, double *out4)
 {
     if (!c || !out4) return fail(SW_ERR_ARG, "sw_stats: NULL argument");
-    unsigned long long h[8];
+    unsigned long long h[SW_NUM_STATS];
     CU_TRY(cudaMemcpyAsync(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CU_TRY(cudaStreamSynchronize(c->stream));
-    for (int k = 0; k < 8; ++k) out4[k] = (double)h[k];
+    for (int k = 0; k < SW_NUM_STATS; ++k) out4[k] = (double)h[k];
     out4[0] = (double)c->stat_sweeps;
     return SW_OK;
 }

@@ -106,6 +106,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     __shared__ uint32_t s_V[TH][NWORD];
     __shared__ uint32_t s_lab[LAB_WORDS];
     __shared__ uint32_t s_edge[TILE_THREADS / 32][EDGE_CAP + 1];   // + dump slot
+    __shared__ uint32_t s_enext[TILE_THREADS / 32];                 // next edge to hand out, per warp
     __shared__ uint32_t s_table[MODEL == 1 ? (2 * 16) * (2 * 16) : 1];
 
     const uint32_t L = (uint32_t)md.L;
@@ -114,6 +115,14 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     const uint32_t tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
     const uint32_t x0 = tx * TW, y0 = ty * TH;
     const uint32_t q2 = 2u * (uint32_t)md.q;
+    // per-phase clocks (lane 0 of every warp), only when the work counters are on: stats[8 + phase]
+    long long ph_t = stats ? clock64() : 0;
+#define SW_PHASE(i)                                                                     \
+    if (stats) {                                                                        \
+        const long long now_ = clock64();                                               \
+        if (lane == 0u) atomicAdd(stats + 8 + (i), (unsigned long long)(now_ - ph_t)); \
+        ph_t = now_;                                                                    \
+    }
     uint32_t m = 0u;
     if (MODEL == 1) {
         for (uint32_t k = tid; k < q2 * q2; k += TILE_THREADS) s_table[k] = md.table[k];
@@ -181,6 +190,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     }
     __syncthreads();
 
+    SW_PHASE(0)
     // bonds that leave the tile: exported for K2, never used by the tile-local graph below
     if (tid < (uint32_t)TH) {
         const uint32_t b = __ballot_sync(0xFFFFFFFFu, (s_H[tid][NWORD - 1] >> 31) & 1u);
@@ -222,7 +232,9 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         epos = incl - n;
     }
     const uint32_t epos0 = epos;
+    if (lane == 0u) s_enext[warp] = 32u;
 
+    SW_PHASE(1)
     // B1: one left-to-right pass over the 32 bit positions (straight-line, no bit searches).  Every run inherits the
     // run above its lowest up-bond (plain store) or becomes its own root; the other up-bonds go to the edge list.
     uint32_t rs = 0u;                                         // start of the current run
@@ -250,6 +262,13 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         }
     }
     __syncthreads();
+    SW_PHASE(2)
+#ifndef SW_RESOLVE_CHUNK
+#define SW_RESOLVE_CHUNK 4
+#endif
+#ifndef SW_B2_HALVE
+#define SW_B2_HALVE 1
+#endif
 #ifndef SW_JUMP_ROUNDS
 #define SW_JUMP_ROUNDS 0
 #endif
@@ -274,14 +293,25 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         const uint32_t ne = etotal < (uint32_t)EDGE_CAP ? etotal : (uint32_t)EDGE_CAP;
         // Every lane walks its own edges at its own pace (one pointer hop of both ends per trip), so a long
         // chain in one lane does not stall the other lanes edge by edge.
+        // Edges are handed out dynamically (per-warp counter), so the lanes stay evenly loaded.
         uint32_t e = lane;
         if (e < ne) {
             volatile uint32_t *vl = s_lab;
             uint32_t v = s_edge[warp][e];
             uint32_t a0 = v & 0xFFFFu, b0 = v >> 16, a = a0, b = b0;
             for (;;) {
-                const uint32_t pa = vl[a], pb = vl[b];
-                if (pa != a || pb != b) { a = pa; b = pb; continue; }
+                uint32_t pa = vl[a], pb = vl[b];
+                if (pa != a || pb != b) {
+#if SW_B2_HALVE
+                    const uint32_t ga = vl[pa], gb = vl[pb];       // path halving: skip one ancestor on each side
+                    if (ga != pa) vl[a] = ga;
+                    if (gb != pb) vl[b] = gb;
+                    a = ga; b = gb;
+#else
+                    a = pa; b = pb;
+#endif
+                    continue;
+                }
                 uint32_t lo = a;
                 if (a != b) {
                     const uint32_t hi = a > b ? a : b;
@@ -291,7 +321,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
                 }
                 if (vl[a0] > lo && a0 != lo) vl[a0] = lo;           // both ends straight to the root (an ancestor)
                 if (vl[b0] > lo && b0 != lo) vl[b0] = lo;
-                e += 32u;
+                e = atomicAdd(&s_enext[warp], 1u);
                 if (e >= ne) break;
                 v = s_edge[warp][e];
                 a0 = v & 0xFFFFu; b0 = v >> 16; a = a0; b = b0;
@@ -311,6 +341,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     }
     __syncthreads();
 
+    SW_PHASE(3)
     // B3: clusters that may continue in another tile: every cluster with a site in the top row or the left column
     // (their bonds belong to the neighbouring tiles), or with an active bond across the right or bottom edge.
     // One boundary site per thread and pass; only the first site of a run (or of a bonded stretch) does the work.
@@ -343,27 +374,41 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     }
     __syncthreads();
 
-    // B4a: resolve every run of the word to its root (+ LOPEN), lane-autonomous: one pointer hop per trip, a lane
-    // moves on to its next run as soon as one is resolved and writes the root back to the run's own entry
+    SW_PHASE(4)
+    // B4a: resolve every run of the word to its root (+ LOPEN).  First a straight-line pass: three pointer hops
+    // for all runs of the word at once (the loads of one level are independent, so their latencies overlap) with
+    // the result written back to the run's own entry; runs deeper than that (rare) are finished by a lane-autonomous
+    // chase that starts from the already advanced pointer.
     uint32_t hops = 0u;
     {
         volatile uint32_t *vl = s_lab;
-        uint32_t rem = S;
-        uint32_t k = 31u - (uint32_t)__clz((int)rem);        // S has bit 0 set
-        uint32_t own = sb + k, a = own;
-        for (;;) {
-            const uint32_t x = vl[a];
-            const uint32_t p = x & LMASK;
-            if (p != a) { a = p; ++hops; continue; }
-            vl[own] = x;
+        uint32_t rem = 0u;
+#pragma unroll
+        for (int c = 0; c < 32; c += SW_RESOLVE_CHUNK) {
+            uint32_t x[SW_RESOLVE_CHUNK], y[SW_RESOLVE_CHUNK];
+#pragma unroll
+            for (int j = 0; j < SW_RESOLVE_CHUNK; ++j) x[j] = ((S >> (c + j)) & 1u) ? vl[sb + c + j] : 0u;
+#pragma unroll
+            for (int j = 0; j < SW_RESOLVE_CHUNK; ++j) if ((S >> (c + j)) & 1u) x[j] = vl[x[j] & LMASK];
+#pragma unroll
+            for (int j = 0; j < SW_RESOLVE_CHUNK; ++j) if ((S >> (c + j)) & 1u) y[j] = vl[x[j] & LMASK];
+#pragma unroll
+            for (int j = 0; j < SW_RESOLVE_CHUNK; ++j)
+                if ((S >> (c + j)) & 1u) {
+                    vl[sb + c + j] = y[j];
+                    if ((y[j] & LMASK) != (x[j] & LMASK)) rem |= 1u << (c + j);
+                }
+        }
+        while (rem) {
+            const uint32_t k = 31u - (uint32_t)__clz((int)rem);
             rem ^= 1u << k;
-            if (!rem) break;
-            k = 31u - (uint32_t)__clz((int)rem);
-            own = sb + k;
-            a = own;
+            uint32_t a = vl[sb + k] & LMASK, v;
+            while (((v = vl[a]) & LMASK) != a) { a = v & LMASK; ++hops; }
+            vl[sb + k] = v;
         }
     }
     __syncwarp();
+    SW_PHASE(5)
 
     // B4b: per-site labels of the word (64 contiguous bytes); open roots enter the global union-find as their
     // own parent
@@ -385,10 +430,16 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         uint4 *dst = reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
 #pragma unroll
         for (int c = 0; c < 4; ++c) dst[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
+        SW_PHASE(6)
         if (stats) {
-            atomicAdd(stats + 2, (unsigned long long)__popc(S));
-            atomicAdd(stats + 3, (unsigned long long)(epos - epos0));
-            atomicAdd(stats + 4, (unsigned long long)hops);
+            const uint32_t n2 = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popc(S));
+            const uint32_t n3 = __reduce_add_sync(0xFFFFFFFFu, epos - epos0);
+            const uint32_t n4 = __reduce_add_sync(0xFFFFFFFFu, hops);
+            if (lane == 0u) {
+                atomicAdd(stats + 2, (unsigned long long)n2);
+                atomicAdd(stats + 3, (unsigned long long)n3);
+                atomicAdd(stats + 4, (unsigned long long)n4);
+            }
         }
     }
 }
