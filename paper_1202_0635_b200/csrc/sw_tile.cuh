@@ -266,6 +266,9 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
 #ifndef SW_RESOLVE_CHUNK
 #define SW_RESOLVE_CHUNK 4
 #endif
+#ifndef SW_B2_ILP
+#define SW_B2_ILP 1
+#endif
 #ifndef SW_B2_HALVE
 #define SW_B2_HALVE 1
 #endif
@@ -291,40 +294,51 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     // B2: the warp's edges, one per lane and round (union-find by minimum index: PAPER.md:47 at tile level)
     {
         const uint32_t ne = etotal < (uint32_t)EDGE_CAP ? etotal : (uint32_t)EDGE_CAP;
-        // Every lane walks its own edges at its own pace (one pointer hop of both ends per trip), so a long
-        // chain in one lane does not stall the other lanes edge by edge.
-        // Edges are handed out dynamically (per-warp counter), so the lanes stay evenly loaded.
-        uint32_t e = lane;
-        if (e < ne) {
-            volatile uint32_t *vl = s_lab;
-            uint32_t v = s_edge[warp][e];
-            uint32_t a0 = v & 0xFFFFu, b0 = v >> 16, a = a0, b = b0;
-            for (;;) {
-                uint32_t pa = vl[a], pb = vl[b];
-                if (pa != a || pb != b) {
+        // Every lane keeps SW_B2_ILP edges in flight: the pointer loads of the edges are independent, so their
+        // shared-memory latencies overlap; a lane leaves the loop when all its edges of the batch are merged.
+        volatile uint32_t *vl = s_lab;
+        for (uint32_t e0 = lane; e0 < ne; e0 += 32u * SW_B2_ILP) {
+            uint32_t a[SW_B2_ILP], b[SW_B2_ILP];
+            uint32_t live = 0u;
+#pragma unroll
+            for (int j = 0; j < SW_B2_ILP; ++j) {
+                const uint32_t e = e0 + 32u * j;
+                a[j] = b[j] = 0u;
+                if (e < ne) {
+                    const uint32_t v = s_edge[warp][e];
+                    a[j] = v & 0xFFFFu; b[j] = v >> 16;
+                    live |= 1u << j;
+                }
+            }
+            while (live) {
+                uint32_t pa[SW_B2_ILP], pb[SW_B2_ILP];
+#pragma unroll
+                for (int j = 0; j < SW_B2_ILP; ++j) { pa[j] = vl[a[j]]; pb[j] = vl[b[j]]; }
 #if SW_B2_HALVE
-                    const uint32_t ga = vl[pa], gb = vl[pb];       // path halving: skip one ancestor on each side
-                    if (ga != pa) vl[a] = ga;
-                    if (gb != pb) vl[b] = gb;
-                    a = ga; b = gb;
-#else
-                    a = pa; b = pb;
+                uint32_t ga[SW_B2_ILP], gb[SW_B2_ILP];
+#pragma unroll
+                for (int j = 0; j < SW_B2_ILP; ++j) { ga[j] = vl[pa[j]]; gb[j] = vl[pb[j]]; }
 #endif
-                    continue;
+#pragma unroll
+                for (int j = 0; j < SW_B2_ILP; ++j) {
+                    if (!((live >> j) & 1u)) continue;
+                    if (pa[j] != a[j] || pb[j] != b[j]) {
+#if SW_B2_HALVE
+                        if (ga[j] != pa[j]) vl[a[j]] = ga[j];     // path halving: skip one ancestor on each side
+                        if (gb[j] != pb[j]) vl[b[j]] = gb[j];
+                        a[j] = ga[j]; b[j] = gb[j];
+#else
+                        a[j] = pa[j]; b[j] = pb[j];
+#endif
+                    } else if (a[j] == b[j]) {
+                        live &= ~(1u << j);
+                    } else {
+                        const uint32_t hi = a[j] > b[j] ? a[j] : b[j], lo = a[j] > b[j] ? b[j] : a[j];
+                        const uint32_t old = atomicMin(s_lab + hi, lo);
+                        if (old == hi) live &= ~(1u << j);
+                        else { a[j] = old; b[j] = lo; }           // hi had a parent already: keep it connected to lo
+                    }
                 }
-                uint32_t lo = a;
-                if (a != b) {
-                    const uint32_t hi = a > b ? a : b;
-                    lo = a > b ? b : a;
-                    const uint32_t old = atomicMin(s_lab + hi, lo);
-                    if (old != hi) { a = old; b = lo; continue; }   // hi had a parent already: keep it connected to lo
-                }
-                if (vl[a0] > lo && a0 != lo) vl[a0] = lo;           // both ends straight to the root (an ancestor)
-                if (vl[b0] > lo && b0 != lo) vl[b0] = lo;
-                e = atomicAdd(&s_enext[warp], 1u);
-                if (e >= ne) break;
-                v = s_edge[warp][e];
-                a0 = v & 0xFFFFu; b0 = v >> 16; a = a0; b = b0;
             }
         }
         if (etotal > (uint32_t)EDGE_CAP && epos > (uint32_t)EDGE_CAP) {
