@@ -3,11 +3,13 @@
 // arithmetic is the threshold table (double precision, once per context; R6/R7).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "sw.h"
@@ -48,7 +50,7 @@ bool args_ok(int L, int q, int model)
 }
 
 struct Carve {
-    size_t spins, labels, bonds, table, obs, flag, stats, ring, tiled, total;
+    size_t spins, spins2, labels, bonds, table, obs, flag, stats, ring, tiled, total;
 };
 
 Carve carve(int L, int q)
@@ -58,6 +60,7 @@ Carve carve(int L, int q)
     Carve c;
     size_t off = 0;
     c.spins = off;  off += align_up(N);
+    c.spins2 = off; off += align_up(N);
     c.labels = off; off += align_up(4 * N);
     c.bonds = off;  off += align_up(N);
     c.table = off;  off += align_up(4 * (size_t)(2 * SW_MAX_Q) * (2 * SW_MAX_Q));
@@ -81,7 +84,7 @@ struct sw_ctx {
     bool own_stream = false, own_ws = false;
     char *ws = nullptr;
     Carve cv{};
-    uint8_t *spins = nullptr, *bonds = nullptr;
+    uint8_t *spins = nullptr, *spins_alt = nullptr, *bonds = nullptr;  // spins = S^t; spins_alt = the other buffer of the tiled ping-pong
     int32_t *labels = nullptr;
     uint32_t *table = nullptr;
     unsigned long long *obs = nullptr, *stats = nullptr, *ring = nullptr;
@@ -155,9 +158,10 @@ int one_sweep(sw_ctx *c, cudaEvent_t *ev = nullptr)
     const uint32_t t = (uint32_t)c->t;
     int rc;
     if (c->algo == SW_ALGO_TILED) {
-        rc = sw::tiled_sweep(c->tiled, c->md, c->key, t, c->spins, c->labels, c->stream, c->stats_on ? c->stats : nullptr,
-                             &c->launches, ev);
+        rc = sw::tiled_sweep(c->tiled, c->md, c->key, t, c->spins, c->spins_alt, c->labels, c->stream,
+                             c->stats_on ? c->stats : nullptr, &c->launches, ev);
         if (rc != 0) return fail(SW_ERR_CUDA, "tiled sweep launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        std::swap(c->spins, c->spins_alt);   // spins_alt now holds S^t, the input of this sweep
     } else {
         rc = generic_sweep(c, t, ev);
     }
@@ -222,6 +226,7 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
         c->stream = (cudaStream_t)stream;
     }
     c->spins = (uint8_t *)(c->ws + c->cv.spins);
+    c->spins_alt = (uint8_t *)(c->ws + c->cv.spins2);
     c->labels = (int32_t *)(c->ws + c->cv.labels);
     c->bonds = (uint8_t *)(c->ws + c->cv.bonds);
     c->table = (uint32_t *)(c->ws + c->cv.table);
@@ -399,10 +404,12 @@ int sw_get_labels(sw_ctx *c, int32_t *host_out)
     if (!c || !host_out) return fail(SW_ERR_ARG, "sw_get_labels: NULL argument");
     if (!c->have_labels) return fail(SW_ERR_ARG, "sw_get_labels: no sweep has been executed on this configuration");
     if (c->last_algo == SW_ALGO_TILED) {
-        // The tiled back-end keeps tile-local labels + a sparse global parent array: resolve into a scratch buffer.
+        // The tiled sweep fuses the decisions of tile-local clusters into its labels, so the canonical roots are
+        // rebuilt from the sweep's input (still in the other ping-pong buffer) and its bonds (sweep index t - 1).
         int32_t *tmp = nullptr;
         CU_TRY(cudaMalloc((void **)&tmp, 4 * c->N));
-        int rc = sw::tiled_resolve_labels(c->tiled, c->md, c->labels, tmp, c->stream, &c->launches);
+        int rc = sw::tiled_relabel(c->tiled, c->md, c->key, (uint32_t)(c->t - 1), c->spins_alt, c->labels, tmp, c->stream,
+                                   &c->launches);
         cudaError_t e = rc == 0 ? cudaMemcpyAsync(host_out, tmp, 4 * c->N, cudaMemcpyDeviceToHost, c->stream) : cudaErrorUnknown;
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
         cudaFree(tmp);

@@ -42,13 +42,19 @@ constexpr uint32_t LMASK = 0x3FFFu;     // local index field of a label
 constexpr uint32_t LOPEN = 0x8000u;     // cluster may continue in another tile
 constexpr int LAB_WORDS = TILE_SITES + TILE_SITES / 32;   // skewed tile-local index sp = p + (p >> 5)
 constexpr int EDGE_CAP = 256;           // union edges listed per warp (more are handled by their own thread)
-static_assert(LAB_WORDS <= (int)LMASK + 1, "skewed local index must fit the label field");
+constexpr int DEC_BASE = LAB_WORDS;     // label values DEC_BASE + d: "closed cluster, decision d" (self-pointing constants)
+constexpr int NDEC = 16;               // decisions are < q <= 16
+constexpr int RCAP = 256;               // closed roots listed per warp for the converged decision draw
+constexpr int OCAP = 512;               // open roots listed per tile (<= 128 + 64 + 128 + 64 boundary positions)
+static_assert(DEC_BASE + NDEC <= (int)LMASK + 1, "skewed local index and the decision constants must fit the label field");
 static_assert((TILE_THREADS / 32) * ROWS_PER_WARP == TH, "phase A row split");
 
 struct TiledState {
     uint16_t *lab16 = nullptr;   // [L][L] tile-local root of every site (+ LOPEN)
     uint32_t *hedge = nullptr;   // [L/128][L/32]  bit (y & 31) of word y >> 5: +x bond of column 128 tx + 127, row y
     uint32_t *vedge = nullptr;   // [L/TH][L/32]   bit (x & 31) of word x >> 5: +y bond of row TH ty + TH - 1, column x
+    uint16_t *olist = nullptr;   // [tiles][OCAP]  skewed tile-local indices of the open roots of every tile
+    uint32_t *ocount = nullptr;  // [tiles]        how many
     int L = 0;
 };
 
@@ -58,7 +64,9 @@ static inline size_t tiled_workspace_bytes(int L)
 {
     if (!tiled_supported(L)) return 0;
     const size_t N = (size_t)L * L;
-    return 2 * N + 1024 + (size_t)(L / TW) * (L / 32) * 4 + 1024 + (size_t)(L / TH) * (L / 32) * 4 + 1024;
+    const size_t tiles = (size_t)(L / TW) * (L / TH);
+    return 2 * N + 1024 + (size_t)(L / TW) * (L / 32) * 4 + 1024 + (size_t)(L / TH) * (L / 32) * 4 + 1024 +
+           tiles * OCAP * 2 + 1024 + tiles * 4 + 1024;
 }
 
 // ---- shared-memory union-find by minimum index (same scheme as uf_union in sw_generic.cuh) ------------------
@@ -92,6 +100,14 @@ __device__ __forceinline__ void sunion(uint32_t *lab, uint32_t a, uint32_t b)
 // first site (bit position) of the segment that holds bit k; S = mask of segment starts (bit 0 always set)
 __device__ __forceinline__ uint32_t seg_start(uint32_t S, uint32_t k) { return 31u - __clz(S & ((2u << k) - 1u)); }
 
+// Global site index of the tile-local root named by label word `v` of a site of the tile with origin (X0, Y0).
+__device__ __forceinline__ uint32_t root_site(uint32_t v, uint32_t X0, uint32_t Y0, uint32_t L)
+{
+    const uint32_t sp = v & LMASK;
+    const uint32_t p = sp - sp / 33u;          // undo the skew sp = p + (p >> 5)
+    return (Y0 + p / TW) * L + X0 + p % TW;
+}
+
 // K1.  grid = tiles, block = TILE_THREADS.  MODEL 0 = Potts, 1 = clock.
 #ifndef SW_LABEL_MINB
 #define SW_LABEL_MINB 5
@@ -100,11 +116,12 @@ template <int MODEL>
 __global__ void __launch_bounds__(TILE_THREADS, SW_LABEL_MINB)
 k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ spins, uint16_t *__restrict__ lab16,
              int32_t *__restrict__ parent, uint32_t *__restrict__ hedge, uint32_t *__restrict__ vedge,
-             unsigned long long *stats)
+             uint16_t *__restrict__ olist, uint32_t *__restrict__ ocount, int fuse, unsigned long long *stats)
 {
     __shared__ uint32_t s_H[TH][NWORD];
     __shared__ uint32_t s_V[TH][NWORD];
-    __shared__ uint32_t s_lab[LAB_WORDS];
+    __shared__ uint32_t s_lab[LAB_WORDS + NDEC];
+    __shared__ uint32_t s_nopen;
     __shared__ uint32_t s_edge[TILE_THREADS / 32][EDGE_CAP + 1];   // + dump slot
     __shared__ uint32_t s_enext[TILE_THREADS / 32];                 // next edge to hand out, per warp
     __shared__ uint32_t s_table[MODEL == 1 ? (2 * 16) * (2 * 16) : 1];
@@ -123,7 +140,12 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         if (lane == 0u) atomicAdd(stats + 8 + (i), (unsigned long long)(now_ - ph_t)); \
         ph_t = now_;                                                                    \
     }
+    uint16_t *const s_olist = reinterpret_cast<uint16_t *>(&s_V[0][0]);   // reused after B3: the tile's open roots
+    static_assert(sizeof(s_V) >= OCAP * sizeof(uint16_t), "open list must fit the V masks");
+    static_assert(2 * (EDGE_CAP + 1) >= RCAP, "closed-root list must fit the warp's edge list");
     uint32_t m = 0u;
+    if (tid < (uint32_t)NDEC) s_lab[DEC_BASE + tid] = DEC_BASE + tid;
+    if (tid == 32u) s_nopen = 0u;
     if (MODEL == 1) {
         for (uint32_t k = tid; k < q2 * q2; k += TILE_THREADS) s_table[k] = md.table[k];
         m = axis_of_sweep(key, t, (uint32_t)md.q);
@@ -389,6 +411,95 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     __syncthreads();
 
     SW_PHASE(4)
+    // B3b: the roots of the tile (S3 for the clusters that end inside the tile).  Only a run without a bond to the
+    // row above can be a root: every other run was given a smaller parent in B1.  `cand` = END bits of such runs
+    // (a carry started at the run start runs along the links of the run while no site has an up-bond and lands on
+    // the end bit).  A root's entry gets its final 16-bit output value in the upper half: open roots sp | LOPEN
+    // (they also join the tile's open list and the global union-find), closed roots DEC_BASE + decision, drawn from
+    // the CLUSTER stream keyed on the root's global site index (R5).
+    {
+        volatile uint32_t *vl = s_lab;
+        const uint32_t g0 = (y0 + wy) * L + x0 + ww * 32u;
+        const uint32_t cend = ((hin & ~u) + (S & ~u)) & ~hin & ~u;
+        // end bits -> start bits: the same carry trick on the bit-reversed word
+        const uint32_t lr = __brev(hin) >> 1;
+        const uint32_t cs = __brev((lr + __brev(cend)) & ~lr);
+        uint32_t rootc = 0u, rooto = 0u;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            if ((cs >> k) & 1u) {
+                const uint32_t v = vl[sb + k];
+                if ((v & LMASK) == sb + (uint32_t)k) {
+                    if (v & LOPEN) rooto |= 1u << k; else rootc |= 1u << k;
+                }
+            }
+        }
+        while (rooto) {
+            const uint32_t k = (uint32_t)__ffs((int)rooto) - 1u;
+            rooto &= rooto - 1u;
+            const uint32_t v = (sb + k) | LOPEN;
+            const uint32_t pos = atomicAdd(&s_nopen, 1u);
+            s_olist[pos] = (uint16_t)(sb + k);
+            parent[g0 + k] = (int32_t)(g0 + k);
+            vl[sb + k] = v | (v << 16);
+        }
+        if (!fuse) {
+            while (rootc) {
+                const uint32_t k = (uint32_t)__ffs((int)rootc) - 1u;
+                rootc &= rootc - 1u;
+                vl[sb + k] = (sb + k) | ((sb + k) << 16);
+            }
+        } else {
+            // compact the warp's closed roots into its list (reusing the second half of the warp's edge list), then
+            // draw the decisions with all lanes busy
+            uint16_t *rl = reinterpret_cast<uint16_t *>(&s_edge[warp][0]) + 2 * (EDGE_CAP + 1) - RCAP;
+            const uint32_t n = __popc(rootc);
+            uint32_t incl = n;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+                if (lane >= (uint32_t)d) incl += o;
+            }
+            const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+            if (total <= (uint32_t)RCAP) {
+                uint32_t at = incl - n;
+                while (rootc) {
+                    const uint32_t k = (uint32_t)__ffs((int)rootc) - 1u;
+                    rootc &= rootc - 1u;
+                    rl[at++] = (uint16_t)(sb + k);
+                }
+                __syncwarp();
+                for (uint32_t i = lane; i < total; i += 32u) {
+                    const uint32_t sp = rl[i];
+                    const uint32_t r = root_site(sp, x0, y0, L);
+                    uint32_t w[4];
+                    philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
+                    const uint32_t wsel = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
+                    const uint32_t out = (uint32_t)DEC_BASE + (MODEL == 0 ? mulhi_q(wsel, (uint32_t)md.q) : (wsel >> 31));
+                    vl[sp] = sp | (out << 16);
+                }
+            } else {
+                while (rootc) {   // more roots than the list holds (hot configurations): every lane draws its own
+                    const uint32_t k = (uint32_t)__ffs((int)rootc) - 1u;
+                    rootc &= rootc - 1u;
+                    const uint32_t r = g0 + k;
+                    uint32_t w[4];
+                    philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
+                    const uint32_t wsel = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
+                    const uint32_t out = (uint32_t)DEC_BASE + (MODEL == 0 ? mulhi_q(wsel, (uint32_t)md.q) : (wsel >> 31));
+                    vl[sb + k] = (sb + k) | (out << 16);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    {
+        const uint32_t no = s_nopen;
+        for (uint32_t i = tid; i < no; i += TILE_THREADS) olist[(size_t)blockIdx.x * OCAP + i] = s_olist[i];
+        if (tid == 0u) ocount[blockIdx.x] = no;
+    }
+
+    SW_PHASE(7)
     // B4a: resolve every run of the word to its root (+ LOPEN).  First a straight-line pass: three pointer hops
     // for all runs of the word at once (the loads of one level are independent, so their latencies overlap) with
     // the result written back to the run's own entry; runs deeper than that (rare) are finished by a lane-autonomous
@@ -424,22 +535,17 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     __syncwarp();
     SW_PHASE(5)
 
-    // B4b: per-site labels of the word (64 contiguous bytes); open roots enter the global union-find as their
-    // own parent
+    // B4b: per-site labels of the word (64 contiguous bytes)
     {
         volatile uint32_t *vl = s_lab;
-        const uint32_t g0 = (y0 + wy) * L + x0 + ww * 32u;
         uint32_t xs[32];
 #pragma unroll
         for (int k = 0; k < 32; ++k) xs[k] = ((S >> k) & 1u) ? vl[sb + k] : 0u;
         uint32_t cur = 0u, o[16];
 #pragma unroll
         for (int k = 0; k < 32; ++k) {
-            if ((S >> k) & 1u) {
-                cur = xs[k];
-                if (cur == ((sb + (uint32_t)k) | LOPEN)) parent[g0 + k] = (int32_t)(g0 + k);
-            }
-            if (k & 1) o[k >> 1] |= cur << 16; else o[k >> 1] = cur;
+            if ((S >> k) & 1u) cur = xs[k];          // upper half = output value of the run's root (B3b)
+            if (k & 1) o[k >> 1] |= cur & 0xFFFF0000u; else o[k >> 1] = cur >> 16;
         }
         uint4 *dst = reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
 #pragma unroll
@@ -456,14 +562,6 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             }
         }
     }
-}
-
-// Global site index of the tile-local root named by label word `v` of a site of the tile with origin (X0, Y0).
-__device__ __forceinline__ uint32_t root_site(uint32_t v, uint32_t X0, uint32_t Y0, uint32_t L)
-{
-    const uint32_t sp = v & LMASK;
-    const uint32_t p = sp - sp / 33u;          // undo the skew sp = p + (p >> 5)
-    return (Y0 + p / TW) * L + X0 + p % TW;
 }
 
 __device__ __forceinline__ uint32_t root_site_of(const uint16_t *__restrict__ lab16, uint32_t x, uint32_t y, uint32_t L)
@@ -516,75 +614,57 @@ k_seam_merge(Model md, const uint32_t *__restrict__ hedge, const uint32_t *__res
     }
 }
 
-// K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).
+// K2b.  grid = tiles.  Every open root is pointed straight at the root of its cluster, so K3 needs one load per
+// open root.  A concurrent reader sees either the old parent or the root: both are ancestors.
+__global__ void __launch_bounds__(128)
+k_open_flatten(Model md, const uint16_t *__restrict__ olist, const uint32_t *__restrict__ ocount, int32_t *parent)
+{
+    const uint32_t L = (uint32_t)md.L;
+    const uint32_t tiles_x = L / TW;
+    const uint32_t x0 = (blockIdx.x % tiles_x) * TW, y0 = (blockIdx.x / tiles_x) * TH;
+    const uint32_t no = ocount[blockIdx.x];
+    for (uint32_t i = threadIdx.x; i < no; i += blockDim.x) {
+        const int32_t r = (int32_t)root_site(olist[(size_t)blockIdx.x * OCAP + i], x0, y0, L);
+        const int32_t a = uf_find(parent, r);
+        if (a != r) parent[r] = a;
+    }
+}
+
+// K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).  in = S^t, out = S^{t+1}.
 template <int MODEL>
 __global__ void __launch_bounds__(TILE_THREADS)
 k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ lab16, const int32_t *__restrict__ parent,
-            uint8_t *__restrict__ spins)
+            const uint16_t *__restrict__ olist, const uint32_t *__restrict__ ocount,
+            const uint8_t *__restrict__ in, uint8_t *__restrict__ out)
 {
     constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
-    __shared__ uint16_t s_roots[TILE_SITES];   // compacted tile-local roots (+ LOPEN)
-    __shared__ uint8_t s_dec[LAB_WORDS];       // decision of the cluster whose tile-local root is sp (skewed index)
-    __shared__ uint32_t s_count;
+    __shared__ uint8_t s_dec[LAB_WORDS + NDEC];   // decision of the open cluster whose tile-local root is sp; constants
 
     const uint32_t L = (uint32_t)md.L;
-    const uint32_t tid = threadIdx.x, lane = tid & 31u;
+    const uint32_t tid = threadIdx.x;
     const uint32_t tiles_x = L / TW;
     const uint32_t tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
     const uint32_t x0 = tx * TW, y0 = ty * TH;
-    if (tid == 0u) s_count = 0u;
 
+    // one decision per open root of the tile (S3; R5 CLUSTER stream), keyed on the global root K2b left
+    // in the open root's parent entry
+    const uint32_t no = ocount[blockIdx.x];
+    uint32_t sp = 0u, r = 0u;
+    if (tid < no) {
+        sp = olist[(size_t)blockIdx.x * OCAP + tid];
+        r = (uint32_t)__ldg(parent + root_site(sp, x0, y0, L));
+    }
     uint4 lab[PASSES];
-    uint32_t rootm = 0u, openm = 0u;   // bit 8c + j: site j of pass c is a tile-local root / an open one
 #pragma unroll
     for (int c = 0; c < PASSES; ++c) {
         const uint32_t p8 = ((uint32_t)c * TILE_THREADS + tid) * 8u;
         lab[c] = *reinterpret_cast<const uint4 *>(lab16 + (size_t)(y0 + p8 / TW) * L + x0 + p8 % TW);
-        const uint32_t w[4] = { lab[c].x, lab[c].y, lab[c].z, lab[c].w };
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const uint32_t v = (w[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
-            if ((v & LMASK) == p8 + (p8 >> 5) + j) {
-                rootm |= 1u << (8 * c + j);
-                if (v & LOPEN) openm |= 1u << (8 * c + j);
-            }
-        }
     }
-    __syncthreads();   // s_count = 0 visible
-
-    // compact the roots of the tile: warp prefix sum of the per-thread counts, one atomic per warp
-    {
-        const uint32_t n = __popc(rootm);
-        uint32_t incl = n;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-            if (lane >= (uint32_t)d) incl += o;
-        }
-        uint32_t wbase = 0u;
-        if (lane == 31u) wbase = atomicAdd(&s_count, incl);
-        wbase = __shfl_sync(0xFFFFFFFFu, wbase, 31);
-        uint32_t at = wbase + incl - n, rm = rootm;
-        while (rm) {
-            const uint32_t k = (uint32_t)__ffs((int)rm) - 1u;
-            rm &= rm - 1u;
-            const uint32_t p8 = ((k >> 3) * TILE_THREADS + tid) * 8u;
-            const uint32_t sp = p8 + (p8 >> 5) + (k & 7u);
-            s_roots[at++] = (uint16_t)(sp | (((openm >> k) & 1u) ? LOPEN : 0u));
-        }
-    }
-    __syncthreads();
-
-    // one decision per root: open roots chase to the global root first (S3; R5 CLUSTER stream)
-    const uint32_t nroots = s_count;
-    for (uint32_t i = tid; i < nroots; i += TILE_THREADS) {
-        const uint32_t e = s_roots[i];
-        const uint32_t sp = e & LMASK;
-        uint32_t r = root_site(sp, x0, y0, L);
-        if (e & LOPEN) {
-            int32_t a = (int32_t)r, pa;
-            while ((pa = __ldg(parent + a)) != a) a = pa;
-            r = (uint32_t)a;
+    if (tid < (uint32_t)NDEC) s_dec[DEC_BASE + tid] = (uint8_t)tid;
+    for (uint32_t i = tid; i < no; i += TILE_THREADS) {
+        if (i >= TILE_THREADS) {
+            sp = olist[(size_t)blockIdx.x * OCAP + i];
+            r = (uint32_t)__ldg(parent + root_site(sp, x0, y0, L));
         }
         uint32_t w[4];
         philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
@@ -599,7 +679,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
 #pragma unroll
     for (int c = 0; c < PASSES; ++c) {
         const uint32_t p8 = ((uint32_t)c * TILE_THREADS + tid) * 8u;
-        uint8_t *dst = spins + (size_t)(y0 + p8 / TW) * L + x0 + p8 % TW;
+        const size_t at = (size_t)(y0 + p8 / TW) * L + x0 + p8 % TW;
         const uint32_t w[4] = { lab[c].x, lab[c].y, lab[c].z, lab[c].w };
         uint32_t d[8];
 #pragma unroll
@@ -609,7 +689,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
             o.x = d[0] | (d[1] << 8) | (d[2] << 16) | (d[3] << 24);
             o.y = d[4] | (d[5] << 8) | (d[6] << 16) | (d[7] << 24);
         } else {
-            const uint2 old = *reinterpret_cast<const uint2 *>(dst);
+            const uint2 old = *reinterpret_cast<const uint2 *>(in + at);
             const uint32_t q = (uint32_t)md.q;
             uint32_t s[8];
 #pragma unroll
@@ -623,7 +703,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
             o.x = s[0] | (s[1] << 8) | (s[2] << 16) | (s[3] << 24);
             o.y = s[4] | (s[5] << 8) | (s[6] << 16) | (s[7] << 24);
         }
-        *reinterpret_cast<uint2 *>(dst) = o;
+        *reinterpret_cast<uint2 *>(out + at) = o;
     }
 }
 
@@ -654,42 +734,65 @@ static inline int tiled_init(TiledState &st, const Model &md, char *ws)
     st.hedge = reinterpret_cast<uint32_t *>(ws + off);
     off += ((L / TW) * (L / 32) * 4 + 1023) / 1024 * 1024;
     st.vedge = reinterpret_cast<uint32_t *>(ws + off);
+    off += ((L / TH) * (L / 32) * 4 + 1023) / 1024 * 1024;
+    const size_t tiles = (L / TW) * (L / TH);
+    st.olist = reinterpret_cast<uint16_t *>(ws + off);
+    off += (tiles * OCAP * 2 + 1023) / 1024 * 1024;
+    st.ocount = reinterpret_cast<uint32_t *>(ws + off);
     return 0;
 }
 
-constexpr int TILED_NUM_KERNELS = 3;
-static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k_seam_merge", "k_tile_flip" };
+constexpr int TILED_NUM_KERNELS = 4;
+static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k_seam_merge", "k_open_flatten", "k_tile_flip" };
 
-// ev (optional): ev[0] is recorded before the first kernel, ev[k+1] after kernel k.
-static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, uint8_t *spins,
-                              int32_t *parent, cudaStream_t stream, unsigned long long *stats, uint64_t *launches,
-                              cudaEvent_t *ev)
+static inline void tiled_launch_label(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
+                                      int32_t *parent, int fuse, cudaStream_t stream, unsigned long long *stats)
+{
+    const uint32_t tiles = ((uint32_t)md.L / TW) * ((uint32_t)md.L / TH);
+    if (md.model == 0)
+        k_tile_label<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.olist,
+                                                            st.ocount, fuse, stats);
+    else
+        k_tile_label<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.olist,
+                                                            st.ocount, fuse, stats);
+}
+
+// One sweep: in = S^t (left untouched), out = S^{t+1}.  ev (optional): ev[0] is recorded before the first kernel,
+// ev[k+1] after kernel k.
+static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
+                              uint8_t *out, int32_t *parent, cudaStream_t stream, unsigned long long *stats,
+                              uint64_t *launches, cudaEvent_t *ev)
 {
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tiles = (L / TW) * (L / TH);
     const uint32_t ne = (L / TW) * L + (L / TH) * L;
     if (ev) cudaEventRecord(ev[0], stream);
-    if (md.model == 0)
-        k_tile_label<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, spins, st.lab16, parent, st.hedge, st.vedge, stats);
-    else
-        k_tile_label<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, spins, st.lab16, parent, st.hedge, st.vedge, stats);
+    tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats);
     if (ev) cudaEventRecord(ev[1], stream);
     k_seam_merge<<<(ne + 255) / 256, 256, 0, stream>>>(md, st.hedge, st.vedge, st.lab16, parent, stats);
     if (ev) cudaEventRecord(ev[2], stream);
-    if (md.model == 0)
-        k_tile_flip<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, st.lab16, parent, spins);
-    else
-        k_tile_flip<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, st.lab16, parent, spins);
+    k_open_flatten<<<tiles, 128, 0, stream>>>(md, st.olist, st.ocount, parent);
     if (ev) cudaEventRecord(ev[3], stream);
-    *launches += 3;
+    if (md.model == 0)
+        k_tile_flip<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, st.lab16, parent, st.olist, st.ocount, in, out);
+    else
+        k_tile_flip<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, st.lab16, parent, st.olist, st.ocount, in, out);
+    if (ev) cudaEventRecord(ev[4], stream);
+    *launches += 4;
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
 }
 
-static inline int tiled_resolve_labels(TiledState &st, const Model &md, const int32_t *parent, int32_t *out,
-                                       cudaStream_t stream, uint64_t *launches)
+// Debug export (sw_get_labels): label the configuration `in` with the bonds of sweep t again, this time keeping the
+// tile-local root of every site (no fused decisions), merge, and resolve every site to its canonical root.
+static inline int tiled_relabel(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
+                                int32_t *parent, int32_t *out, cudaStream_t stream, uint64_t *launches)
 {
+    const uint32_t L = (uint32_t)md.L;
+    const uint32_t ne = (L / TW) * L + (L / TH) * L;
+    tiled_launch_label(st, md, key, t, in, parent, 0, stream, nullptr);
+    k_seam_merge<<<(ne + 255) / 256, 256, 0, stream>>>(md, st.hedge, st.vedge, st.lab16, parent, nullptr);
     k_resolve_labels<<<(md.N + 255) / 256, 256, 0, stream>>>(md, st.lab16, parent, out);
-    *launches += 1;
+    *launches += 3;
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
 }
 
