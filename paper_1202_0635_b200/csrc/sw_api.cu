@@ -158,7 +158,7 @@ int one_sweep(sw_ctx *c, cudaEvent_t *ev = nullptr)
     const uint32_t t = (uint32_t)c->t;
     int rc;
     if (c->algo == SW_ALGO_TILED) {
-        rc = sw::tiled_sweep(c->tiled, c->md, c->key, t, c->spins, c->spins_alt, c->labels, c->stream,
+        rc = sw::tiled_sweep(c->tiled, c->md, c->key, t, c->spins, c->spins_alt, (unsigned long long *)c->labels, c->stream,
                              c->stats_on ? c->stats : nullptr, &c->launches, ev);
         if (rc != 0) return fail(SW_ERR_CUDA, "tiled sweep launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         std::swap(c->spins, c->spins_alt);   // spins_alt now holds S^t, the input of this sweep
@@ -408,7 +408,7 @@ int sw_get_labels(sw_ctx *c, int32_t *host_out)
         // rebuilt from the sweep's input (still in the other ping-pong buffer) and its bonds (sweep index t - 1).
         int32_t *tmp = nullptr;
         CU_TRY(cudaMalloc((void **)&tmp, 4 * c->N));
-        int rc = sw::tiled_relabel(c->tiled, c->md, c->key, (uint32_t)(c->t - 1), c->spins_alt, c->labels, tmp, c->stream,
+        int rc = sw::tiled_relabel(c->tiled, c->md, c->key, (uint32_t)(c->t - 1), c->spins_alt, (unsigned long long *)c->labels, tmp, c->stream,
                                    &c->launches);
         cudaError_t e = rc == 0 ? cudaMemcpyAsync(host_out, tmp, 4 * c->N, cudaMemcpyDeviceToHost, c->stream) : cudaErrorUnknown;
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);

@@ -42,18 +42,19 @@ constexpr uint32_t LMASK = 0x3FFFu;     // local index field of a label
 constexpr uint32_t LOPEN = 0x8000u;     // cluster may continue in another tile
 constexpr int LAB_WORDS = TILE_SITES + TILE_SITES / 32;   // skewed tile-local index sp = p + (p >> 5)
 constexpr int EDGE_CAP = 256;           // union edges listed per warp (more are handled by their own thread)
-constexpr int DEC_BASE = LAB_WORDS;     // label values DEC_BASE + d: "closed cluster, decision d" (self-pointing constants)
 constexpr int NDEC = 16;               // decisions are < q <= 16
 constexpr int RCAP = 256;               // closed roots listed per warp for the converged decision draw
+constexpr int DEC_BASE = 512;           // lab16 value DEC_BASE + d: "closed cluster, decision d" (= OCAP)
+constexpr int ECNT = 2 * TH + 2 * TW;     // edge labels exported per tile: left column, right column, top row, bottom row
 constexpr int OCAP = 512;               // open roots listed per tile (<= 128 + 64 + 128 + 64 boundary positions)
-static_assert(DEC_BASE + NDEC <= (int)LMASK + 1, "skewed local index and the decision constants must fit the label field");
+static_assert(LAB_WORDS <= (int)LMASK + 1, "skewed local index must fit the label field");
 static_assert((TILE_THREADS / 32) * ROWS_PER_WARP == TH, "phase A row split");
 
 struct TiledState {
     uint16_t *lab16 = nullptr;   // [L][L] tile-local root of every site (+ LOPEN)
     uint32_t *hedge = nullptr;   // [L/128][L/32]  bit (y & 31) of word y >> 5: +x bond of column 128 tx + 127, row y
     uint32_t *vedge = nullptr;   // [L/TH][L/32]   bit (x & 31) of word x >> 5: +y bond of row TH ty + TH - 1, column x
-    uint16_t *olist = nullptr;   // [tiles][OCAP]  skewed tile-local indices of the open roots of every tile
+    uint16_t *edges = nullptr;   // [tiles][ECNT]  lab16 values of the tile's boundary sites: left col, right col, top row, bottom row
     uint32_t *ocount = nullptr;  // [tiles]        how many
     int L = 0;
 };
@@ -66,7 +67,31 @@ static inline size_t tiled_workspace_bytes(int L)
     const size_t N = (size_t)L * L;
     const size_t tiles = (size_t)(L / TW) * (L / TH);
     return 2 * N + 1024 + (size_t)(L / TW) * (L / 32) * 4 + 1024 + (size_t)(L / TH) * (L / 32) * 4 + 1024 +
-           tiles * OCAP * 2 + 1024 + tiles * 4 + 1024;
+           tiles * ECNT * 2 + 1024 + tiles * 4 + 1024;
+}
+
+// Programmatic dependent launch: every kernel of the sweep lets the next one be scheduled early (its CTAs become
+// resident while this grid drains) and itself waits here until the previous grid has completed and flushed.
+__device__ __forceinline__ void pdl_prologue()
+{
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
+template <typename... Params, typename... Args>
+static inline void launch_pdl(void (*kernel)(Params...), unsigned grid, unsigned block, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
 }
 
 // ---- shared-memory union-find by minimum index (same scheme as uf_union in sw_generic.cuh) ------------------
@@ -115,17 +140,18 @@ __device__ __forceinline__ uint32_t root_site(uint32_t v, uint32_t X0, uint32_t 
 template <int MODEL>
 __global__ void __launch_bounds__(TILE_THREADS, SW_LABEL_MINB)
 k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ spins, uint16_t *__restrict__ lab16,
-             int32_t *__restrict__ parent, uint32_t *__restrict__ hedge, uint32_t *__restrict__ vedge,
-             uint16_t *__restrict__ olist, uint32_t *__restrict__ ocount, int fuse, unsigned long long *stats)
+             unsigned long long *__restrict__ parent, uint32_t *__restrict__ hedge, uint32_t *__restrict__ vedge,
+             uint16_t *__restrict__ edges, uint32_t *__restrict__ ocount, int fuse, unsigned long long *stats)
 {
     __shared__ uint32_t s_H[TH][NWORD];
     __shared__ uint32_t s_V[TH][NWORD];
-    __shared__ uint32_t s_lab[LAB_WORDS + NDEC];
+    __shared__ uint32_t s_lab[LAB_WORDS];
     __shared__ uint32_t s_nopen;
     __shared__ uint32_t s_edge[TILE_THREADS / 32][EDGE_CAP + 1];   // + dump slot
     __shared__ uint32_t s_enext[TILE_THREADS / 32];                 // next edge to hand out, per warp
     __shared__ uint32_t s_table[MODEL == 1 ? (2 * 16) * (2 * 16) : 1];
 
+    pdl_prologue();
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t tiles_x = L / TW;
@@ -140,11 +166,8 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         if (lane == 0u) atomicAdd(stats + 8 + (i), (unsigned long long)(now_ - ph_t)); \
         ph_t = now_;                                                                    \
     }
-    uint16_t *const s_olist = reinterpret_cast<uint16_t *>(&s_V[0][0]);   // reused after B3: the tile's open roots
-    static_assert(sizeof(s_V) >= OCAP * sizeof(uint16_t), "open list must fit the V masks");
     static_assert(2 * (EDGE_CAP + 1) >= RCAP, "closed-root list must fit the warp's edge list");
     uint32_t m = 0u;
-    if (tid < (uint32_t)NDEC) s_lab[DEC_BASE + tid] = DEC_BASE + tid;
     if (tid == 32u) s_nopen = 0u;
     if (MODEL == 1) {
         for (uint32_t k = tid; k < q2 * q2; k += TILE_THREADS) s_table[k] = md.table[k];
@@ -229,7 +252,6 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     const uint32_t h = s_H[wy][ww];
     const uint32_t hin = h & 0x7FFFFFFFu;                     // bonds inside the word
     const uint32_t S = ~(hin << 1);                           // run starts (bit 0 always)
-    const uint32_t E = ~hin;                                  // run ends (bit 31 always)
     uint32_t u = 0u, ha = 0u;                                 // bonds to the row above / its in-word bonds
     if (wy > 0u) { u = s_V[wy - 1][ww]; ha = s_H[wy - 1][ww] & 0x7FFFFFFFu; }
     const uint32_t Sa = ~(ha << 1);
@@ -257,29 +279,34 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     if (lane == 0u) s_enext[warp] = 32u;
 
     SW_PHASE(1)
-    // B1: one left-to-right pass over the 32 bit positions (straight-line, no bit searches).  Every run inherits the
-    // run above its lowest up-bond (plain store) or becomes its own root; the other up-bonds go to the edge list.
-    uint32_t rs = 0u;                                         // start of the current run
+    // B1: loops over set bits only.  Every run with a bond to the row above inherits (plain store) the run above its
+    // lowest up-bond; a run without one becomes its own root; the other up-bonds go to the warp's edge list.
+    // cs = start bits of the runs without an up-bond: a carry started at the run start runs along the links of the
+    // run while no site has an up-bond and lands on the end bit; the same trick on the reversed word maps end bits
+    // to start bits.
+    uint32_t cs;
     {
-        uint32_t as = 0u, tgt = 132u;                         // start of the run above; target relative to sbu
+        const uint32_t cend = ((hin & ~u) + (S & ~u)) & ~hin & ~u;
+        const uint32_t lr = __brev(hin) >> 1;
+        cs = __brev((lr + __brev(cend)) & ~lr);
+    }
+    {
         uint32_t *el = s_edge[warp];
-#pragma unroll
-        for (int k = 0; k < 32; ++k) {
-            const uint32_t bit = 1u << k;
-            if (Sa & bit) as = (uint32_t)k;
-            if (S & bit) { rs = (uint32_t)k; tgt = 132u + (uint32_t)k; }
-            if (first & bit) tgt = as;
-            {   // listed edge, or a store to the dump slot EDGE_CAP (branch-free)
-                const uint32_t isx = (X >> k) & 1u;
-                uint32_t slot = isx ? epos : (uint32_t)EDGE_CAP;
-                slot = slot < (uint32_t)EDGE_CAP ? slot : (uint32_t)EDGE_CAP;
-                el[slot] = (sb + rs) | ((sbu + as) << 16);
-                epos += isx;
-            }
-            if (E & bit) s_lab[sb + rs] = sbu + tgt;
+        for (uint32_t c = cs; c; c &= c - 1u) {
+            const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
+            s_lab[sb + k] = sb + k;
+        }
+        for (uint32_t f = first; f; f &= f - 1u) {
+            const uint32_t k = (uint32_t)__ffs((int)f) - 1u;
+            s_lab[sb + seg_start(S, k)] = sbu + seg_start(Sa, k);
+        }
+        for (uint32_t xr = X; xr; xr &= xr - 1u) {
+            const uint32_t k = (uint32_t)__ffs((int)xr) - 1u;
+            if (epos < (uint32_t)EDGE_CAP) el[epos] = (sb + seg_start(S, k)) | ((sbu + seg_start(Sa, k)) << 16);
+            ++epos;
         }
         if (hedge_out) {                                      // bond to the next word of the row
-            if (epos < (uint32_t)EDGE_CAP) el[epos] = (sb + 33u) | ((sb + rs) << 16);
+            if (epos < (uint32_t)EDGE_CAP) el[epos] = (sb + 33u) | ((sb + seg_start(S, 31u)) << 16);
             ++epos;
         }
     }
@@ -300,18 +327,28 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
 #ifndef SW_B4_WRITEBACK
 #define SW_B4_WRITEBACK 1
 #endif
-    // B1b: pointer jumping on the inheritance forest (straight-line, all loads of a round independent)
+    // B1b: pointer jumping on the inheritance forest (plain stores only so far: any ancestor is a valid parent, so the
+    // rounds need no barrier between them).  Shallow trees make the finds of B2 and the resolve pass of B4a short.
 #pragma unroll 1
     for (int r = 0; r < SW_JUMP_ROUNDS; ++r) {
-        uint32_t pp[32];
+        volatile uint32_t *vl = s_lab;
+        uint32_t sr = S & ~cs;                                 // runs that inherited
+        while (sr) {
+            uint32_t kk[4], x[4];
 #pragma unroll
-        for (int k = 0; k < 32; ++k) pp[k] = ((S >> k) & 1u) ? s_lab[sb + k] : 0u;
+            for (int j = 0; j < 4; ++j) {
+                kk[j] = sr ? (uint32_t)__ffs((int)sr) - 1u : kk[0];
+                sr &= sr - 1u;
+            }
 #pragma unroll
-        for (int k = 0; k < 32; ++k) if ((S >> k) & 1u) pp[k] = s_lab[pp[k]];
+            for (int j = 0; j < 4; ++j) x[j] = vl[sb + kk[j]];
 #pragma unroll
-        for (int k = 0; k < 32; ++k) if ((S >> k) & 1u) s_lab[sb + k] = pp[k];
-        __syncthreads();
+            for (int j = 0; j < 4; ++j) x[j] = vl[x[j]];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) vl[sb + kk[j]] = x[j];
+        }
     }
+    if (SW_JUMP_ROUNDS > 0) __syncthreads();
 
     // B2: the warp's edges, one per lane and round (union-find by minimum index: PAPER.md:47 at tile level)
     {
@@ -372,7 +409,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
                 if (slot >= (uint32_t)EDGE_CAP) sunion(s_lab, sb + seg_start(S, k), sbu + seg_start(Sa, k));
                 ++slot;
             }
-            if (hedge_out && slot >= (uint32_t)EDGE_CAP) sunion(s_lab, sb + 33u, sb + rs);
+            if (hedge_out && slot >= (uint32_t)EDGE_CAP) sunion(s_lab, sb + 33u, sb + seg_start(S, 31u));
         }
     }
     __syncthreads();
@@ -419,110 +456,96 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     // the CLUSTER stream keyed on the root's global site index (R5).
     {
         volatile uint32_t *vl = s_lab;
-        const uint32_t g0 = (y0 + wy) * L + x0 + ww * 32u;
-        const uint32_t cend = ((hin & ~u) + (S & ~u)) & ~hin & ~u;
-        // end bits -> start bits: the same carry trick on the bit-reversed word
-        const uint32_t lr = __brev(hin) >> 1;
-        const uint32_t cs = __brev((lr + __brev(cend)) & ~lr);
         uint32_t rootc = 0u, rooto = 0u;
-#pragma unroll
-        for (int k = 0; k < 32; ++k) {
-            if ((cs >> k) & 1u) {
-                const uint32_t v = vl[sb + k];
-                if ((v & LMASK) == sb + (uint32_t)k) {
-                    if (v & LOPEN) rooto |= 1u << k; else rootc |= 1u << k;
-                }
+        for (uint32_t c = cs; c; c &= c - 1u) {
+            const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
+            const uint32_t v = vl[sb + k];
+            if ((v & LMASK) == sb + k) {
+                if (v & LOPEN) rooto |= 1u << k; else rootc |= 1u << k;
             }
         }
-        while (rooto) {
-            const uint32_t k = (uint32_t)__ffs((int)rooto) - 1u;
-            rooto &= rooto - 1u;
-            const uint32_t v = (sb + k) | LOPEN;
-            const uint32_t pos = atomicAdd(&s_nopen, 1u);
-            s_olist[pos] = (uint16_t)(sb + k);
-            parent[g0 + k] = (int32_t)(g0 + k);
-            vl[sb + k] = v | (v << 16);
-        }
-        if (!fuse) {
-            while (rootc) {
-                const uint32_t k = (uint32_t)__ffs((int)rootc) - 1u;
-                rootc &= rootc - 1u;
-                vl[sb + k] = (sb + k) | ((sb + k) << 16);
-            }
-        } else {
-            // compact the warp's closed roots into its list (reusing the second half of the warp's edge list), then
-            // draw the decisions with all lanes busy
-            uint16_t *rl = reinterpret_cast<uint16_t *>(&s_edge[warp][0]) + 2 * (EDGE_CAP + 1) - RCAP;
-            const uint32_t n = __popc(rootc);
-            uint32_t incl = n;
+        // compact the warp's roots into its list (reusing the second half of the warp's edge list), so that the
+        // decisions are drawn -- and the open roots registered -- with all lanes busy
+        uint16_t *rl = reinterpret_cast<uint16_t *>(&s_edge[warp][0]) + 2 * (EDGE_CAP + 1) - RCAP;
+        const uint32_t rall = rootc | rooto;
+        const uint32_t n = __popc(rall);
+        uint32_t incl = n;
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-                if (lane >= (uint32_t)d) incl += o;
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+            if (lane >= (uint32_t)d) incl += o;
+        }
+        const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        const bool listed = total <= (uint32_t)RCAP;
+        if (listed) {
+            uint32_t at = incl - n;
+            for (uint32_t rr = rall; rr; rr &= rr - 1u) {
+                const uint32_t k = (uint32_t)__ffs((int)rr) - 1u;
+                rl[at++] = (uint16_t)((sb + k) | (((rooto >> k) & 1u) ? LOPEN : 0u));
             }
-            const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-            if (total <= (uint32_t)RCAP) {
-                uint32_t at = incl - n;
-                while (rootc) {
-                    const uint32_t k = (uint32_t)__ffs((int)rootc) - 1u;
-                    rootc &= rootc - 1u;
-                    rl[at++] = (uint16_t)(sb + k);
-                }
-                __syncwarp();
-                for (uint32_t i = lane; i < total; i += 32u) {
-                    const uint32_t sp = rl[i];
-                    const uint32_t r = root_site(sp, x0, y0, L);
-                    uint32_t w[4];
-                    philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
-                    const uint32_t wsel = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
-                    const uint32_t out = (uint32_t)DEC_BASE + (MODEL == 0 ? mulhi_q(wsel, (uint32_t)md.q) : (wsel >> 31));
-                    vl[sp] = sp | (out << 16);
-                }
+            __syncwarp();
+        }
+        // listed: entry i of the warp's list; else (more roots than the list holds: hot configurations) every lane
+        // walks its own roots
+        uint32_t mine = rall;
+        for (uint32_t i = lane; listed ? (i < total) : (mine != 0u); i += 32u) {
+            uint32_t e;
+            if (listed) {
+                e = rl[i];
             } else {
-                while (rootc) {   // more roots than the list holds (hot configurations): every lane draws its own
-                    const uint32_t k = (uint32_t)__ffs((int)rootc) - 1u;
-                    rootc &= rootc - 1u;
-                    const uint32_t r = g0 + k;
-                    uint32_t w[4];
-                    philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
-                    const uint32_t wsel = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
-                    const uint32_t out = (uint32_t)DEC_BASE + (MODEL == 0 ? mulhi_q(wsel, (uint32_t)md.q) : (wsel >> 31));
-                    vl[sb + k] = (sb + k) | (out << 16);
-                }
+                const uint32_t k = (uint32_t)__ffs((int)mine) - 1u;
+                mine &= mine - 1u;
+                e = (sb + k) | (((rooto >> k) & 1u) ? LOPEN : 0u);
             }
+            const uint32_t sp = e & LMASK;
+            const uint32_t r = root_site(sp, x0, y0, L);
+            uint32_t out = e;
+            if (e & LOPEN) {
+                // open root: node blockIdx.x * OCAP + pos of the global union-find, its own parent; key = (site, node)
+                const uint32_t pos = atomicAdd(&s_nopen, 1u);
+                const uint32_t node = blockIdx.x * (uint32_t)OCAP + pos;
+                parent[node] = ((unsigned long long)r << 32) | node;
+                out = LOPEN | pos;
+            } else if (fuse) {
+                uint32_t w[4];
+                philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
+                const uint32_t wsel = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
+                out = (uint32_t)DEC_BASE + (MODEL == 0 ? mulhi_q(wsel, (uint32_t)md.q) : (wsel >> 31));
+            }
+            vl[sp] = sp | (out << 16);
         }
     }
     __syncthreads();
-    {
-        const uint32_t no = s_nopen;
-        for (uint32_t i = tid; i < no; i += TILE_THREADS) olist[(size_t)blockIdx.x * OCAP + i] = s_olist[i];
-        if (tid == 0u) ocount[blockIdx.x] = no;
-    }
+    if (tid == 0u) ocount[blockIdx.x] = s_nopen;
 
     SW_PHASE(7)
-    // B4a: resolve every run of the word to its root (+ LOPEN).  First a straight-line pass: three pointer hops
-    // for all runs of the word at once (the loads of one level are independent, so their latencies overlap) with
-    // the result written back to the run's own entry; runs deeper than that (rare) are finished by a lane-autonomous
-    // chase that starts from the already advanced pointer.
+    // B4a: resolve every run of the word to its root's entry (whose upper half is the output value).  Four runs at
+    // a time, three pointer hops each (the loads of one level are independent, so their latencies overlap), result
+    // written back to the run's own entry; runs deeper than that (rare) are finished by a chase that starts from the
+    // already advanced pointer.
     uint32_t hops = 0u;
     {
         volatile uint32_t *vl = s_lab;
         uint32_t rem = 0u;
+        uint32_t sr = S;
+        while (sr) {
+            uint32_t kk[4], x[4], y[4];
 #pragma unroll
-        for (int c = 0; c < 32; c += SW_RESOLVE_CHUNK) {
-            uint32_t x[SW_RESOLVE_CHUNK], y[SW_RESOLVE_CHUNK];
+            for (int j = 0; j < 4; ++j) {
+                kk[j] = sr ? (uint32_t)__ffs((int)sr) - 1u : kk[0];
+                sr &= sr - 1u;
+            }
 #pragma unroll
-            for (int j = 0; j < SW_RESOLVE_CHUNK; ++j) x[j] = ((S >> (c + j)) & 1u) ? vl[sb + c + j] : 0u;
+            for (int j = 0; j < 4; ++j) x[j] = vl[sb + kk[j]];
 #pragma unroll
-            for (int j = 0; j < SW_RESOLVE_CHUNK; ++j) if ((S >> (c + j)) & 1u) x[j] = vl[x[j] & LMASK];
+            for (int j = 0; j < 4; ++j) x[j] = vl[x[j] & LMASK];
 #pragma unroll
-            for (int j = 0; j < SW_RESOLVE_CHUNK; ++j) if ((S >> (c + j)) & 1u) y[j] = vl[x[j] & LMASK];
+            for (int j = 0; j < 4; ++j) y[j] = vl[x[j] & LMASK];
 #pragma unroll
-            for (int j = 0; j < SW_RESOLVE_CHUNK; ++j)
-                if ((S >> (c + j)) & 1u) {
-                    vl[sb + c + j] = y[j];
-                    if ((y[j] & LMASK) != (x[j] & LMASK)) rem |= 1u << (c + j);
-                }
+            for (int j = 0; j < 4; ++j) {
+                vl[sb + kk[j]] = y[j];
+                if ((y[j] ^ x[j]) & LMASK) rem |= 1u << kk[j];
+            }
         }
         while (rem) {
             const uint32_t k = 31u - (uint32_t)__clz((int)rem);
@@ -550,6 +573,15 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         uint4 *dst = reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
 #pragma unroll
         for (int c = 0; c < 4; ++c) dst[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
+        // the labels of the tile's boundary sites, compact, for K2
+        uint16_t *ed = edges + (size_t)blockIdx.x * ECNT;
+        if (ww == 0u) ed[wy] = (uint16_t)o[0];
+        if (ww == (uint32_t)NWORD - 1u) ed[TH + wy] = (uint16_t)(o[15] >> 16);
+        if (wy == 0u || wy == (uint32_t)TH - 1u) {
+            uint4 *de = reinterpret_cast<uint4 *>(ed + 2 * TH + (wy ? TW : 0) + ww * 32u);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) de[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
+        }
         SW_PHASE(6)
         if (stats) {
             const uint32_t n2 = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popc(S));
@@ -564,81 +596,104 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     }
 }
 
-__device__ __forceinline__ uint32_t root_site_of(const uint16_t *__restrict__ lab16, uint32_t x, uint32_t y, uint32_t L)
+// ---- global union-find over the open roots ------------------------------------------------------------------------
+// Node n = tile * OCAP + pos.  parent[n] = key of n's parent, key(m) = (site index of m) << 32 | m; a root holds its own
+// key.  Keys order the nodes by site index, so hooking the larger root under the smaller one (64-bit atomicMin) makes the
+// root of every cluster its minimum site index: the "proper label ... smallest" of PAPER.md:47.  Parents only ever
+// decrease, so a stale read is still an ancestor and the atomicMin re-validates the root.
+__device__ __forceinline__ unsigned long long gfind(unsigned long long *parent, uint32_t x)
 {
-    return root_site(lab16[(size_t)y * L + x], x - x % TW, y - y % TH, L);
+#ifndef SW_SEAM_EXP
+#define SW_SEAM_EXP 0
+#endif
+#if SW_SEAM_EXP == 3
+#define GLD(p_) __ldcg(p_)
+#else
+#define GLD(p_) (*(p_))
+#endif
+    unsigned long long p = GLD(parent + x);
+    uint32_t prev = x;
+    while ((uint32_t)p != prev) {
+        const uint32_t cur = (uint32_t)p;
+        const unsigned long long g = GLD(parent + cur);
+        if ((uint32_t)g == cur) return g;
+        if (SW_SEAM_EXP != 2) parent[prev] = g;                     // path halving
+        prev = cur;
+        p = g;
+    }
+    return p;
 }
 
-// Tile-crossing bond e -> (active, tile-local roots a and b of its two ends, as global site indices).
-// First the (L/128)*L right-edge bonds, then the (L/TH)*L bottom-edge bonds.
-__device__ __forceinline__ bool seam_bond(uint32_t e, uint32_t L, const uint32_t *__restrict__ hedge,
-                                          const uint32_t *__restrict__ vedge, const uint16_t *__restrict__ lab16,
-                                          uint32_t &a, uint32_t &b)
+__device__ __forceinline__ void gunion(unsigned long long *parent, uint32_t x, uint32_t y)
 {
-    const uint32_t nh = (L / TW) * L;
+    for (;;) {
+        unsigned long long kx = gfind(parent, x), ky = gfind(parent, y);
+        if (kx == ky) return;
+        if (kx < ky) { const unsigned long long tmp = kx; kx = ky; ky = tmp; }
+        const unsigned long long old = atomicMin(parent + (uint32_t)kx, ky);   // kx > ky
+        if (old == kx) return;                // kx was a root and now hangs under ky
+        x = (uint32_t)old;                    // kx already had a parent: keep that parent connected to ky
+        y = (uint32_t)ky;
+    }
+}
+
+// read-only find (K3, label export): site index of the root of node x
+__device__ __forceinline__ uint32_t groot_site(const unsigned long long *__restrict__ parent, uint32_t x)
+{
+    unsigned long long p = __ldcg(parent + x);
+    while ((uint32_t)p != x) { x = (uint32_t)p; p = __ldcg(parent + x); }
+    return (uint32_t)(p >> 32);
+}
+
+// K2.  One thread per tile-edge bond position: first the (L/128)*L right-edge bonds, then the (L/TH)*L bottom-edge
+// bonds.  The two ends of an active tile-crossing bond lie in open clusters; their lab16 values (LOPEN | pos) come
+// from the compact edge arrays K1 wrote.
+#ifndef SW_SEAM_BS
+#define SW_SEAM_BS 256
+#endif
+__global__ void __launch_bounds__(SW_SEAM_BS)
+k_seam_merge(Model md, const uint32_t *__restrict__ hedge, const uint32_t *__restrict__ vedge,
+             const uint16_t *__restrict__ edges, unsigned long long *parent, unsigned long long *stats)
+{
+    const uint32_t L = (uint32_t)md.L;
+    const uint32_t tiles_x = L / TW, tiles_y = L / TH;
+    const uint32_t nh = tiles_x * L, ne = nh + tiles_y * L;
+    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_prologue();
+    if (e >= ne) return;
+    uint32_t bit, ta, tb, ia, ib;
     if (e < nh) {
         const uint32_t tx = e / L, y = e - tx * L;
-        if (!((hedge[tx * (L / 32) + (y >> 5)] >> (y & 31u)) & 1u)) return false;
-        const uint32_t x = tx * TW + TW - 1u;
-        const uint32_t xr = (x + 1u == L) ? 0u : x + 1u;
-        a = root_site_of(lab16, x, y, L);
-        b = root_site_of(lab16, xr, y, L);
-        return true;
+        bit = (hedge[tx * (L / 32) + (y >> 5)] >> (y & 31u)) & 1u;
+        ta = (y / TH) * tiles_x + tx;
+        tb = (y / TH) * tiles_x + (tx + 1u == tiles_x ? 0u : tx + 1u);
+        ia = TH + y % TH;                     // right column of ta
+        ib = y % TH;                          // left column of tb
+    } else {
+        const uint32_t f = e - nh;
+        const uint32_t ty = f / L, x = f - ty * L;
+        bit = (vedge[ty * (L / 32) + (x >> 5)] >> (x & 31u)) & 1u;
+        ta = ty * tiles_x + x / TW;
+        tb = (ty + 1u == tiles_y ? 0u : ty + 1u) * tiles_x + x / TW;
+        ia = 2 * TH + TW + x % TW;            // bottom row of ta
+        ib = 2 * TH + x % TW;                 // top row of tb
     }
-    const uint32_t f = e - nh;
-    const uint32_t ty = f / L, x = f - ty * L;
-    if (!((vedge[ty * (L / 32) + (x >> 5)] >> (x & 31u)) & 1u)) return false;
-    const uint32_t y = ty * TH + TH - 1u;
-    const uint32_t yd = (y + 1u == L) ? 0u : y + 1u;
-    a = root_site_of(lab16, x, y, L);
-    b = root_site_of(lab16, x, yd, L);
-    return true;
-}
-
-// K2.  One thread per tile-edge bond position.
-__global__ void __launch_bounds__(256)
-k_seam_merge(Model md, const uint32_t *__restrict__ hedge, const uint32_t *__restrict__ vedge,
-             const uint16_t *__restrict__ lab16, int32_t *parent, unsigned long long *stats)
-{
-    const uint32_t L = (uint32_t)md.L;
-    const uint32_t ne = (L / TW) * L + (L / TH) * L;
-    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t a = 0xFFFFFFFFu, b = 0xFFFFFFFFu;
-    const bool act = (e < ne) && seam_bond(e, L, hedge, vedge, lab16, a, b);
-    // the neighbouring edge position often joins the same pair of tile-local clusters: skip the repeat
-    const uint32_t pa = __shfl_up_sync(0xFFFFFFFFu, a, 1), pb = __shfl_up_sync(0xFFFFFFFFu, b, 1);
-    const bool dup = (threadIdx.x & 31u) != 0u && pa == a && pb == b;
-    if (act && !dup) {
-        if (stats) atomicAdd(stats + 1, 1ull);
-        uf_union(parent, (int32_t)a, (int32_t)b);
-    }
-}
-
-// K2b.  grid = tiles.  Every open root is pointed straight at the root of its cluster, so K3 needs one load per
-// open root.  A concurrent reader sees either the old parent or the root: both are ancestors.
-__global__ void __launch_bounds__(128)
-k_open_flatten(Model md, const uint16_t *__restrict__ olist, const uint32_t *__restrict__ ocount, int32_t *parent)
-{
-    const uint32_t L = (uint32_t)md.L;
-    const uint32_t tiles_x = L / TW;
-    const uint32_t x0 = (blockIdx.x % tiles_x) * TW, y0 = (blockIdx.x / tiles_x) * TH;
-    const uint32_t no = ocount[blockIdx.x];
-    for (uint32_t i = threadIdx.x; i < no; i += blockDim.x) {
-        const int32_t r = (int32_t)root_site(olist[(size_t)blockIdx.x * OCAP + i], x0, y0, L);
-        const int32_t a = uf_find(parent, r);
-        if (a != r) parent[r] = a;
-    }
+    const uint32_t a = edges[(size_t)ta * ECNT + ia], b = edges[(size_t)tb * ECNT + ib];
+    if (!bit) return;
+    if (stats) atomicAdd(stats + 1, 1ull);
+    if (SW_SEAM_EXP == 1) { if (a == 0xFFFFu && b == 0xFFFEu) parent[0] = 0; return; }
+    gunion(parent, ta * OCAP + (a & (OCAP - 1u)), tb * OCAP + (b & (OCAP - 1u)));
 }
 
 // K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).  in = S^t, out = S^{t+1}.
 template <int MODEL>
 __global__ void __launch_bounds__(TILE_THREADS)
-k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ lab16, const int32_t *__restrict__ parent,
-            const uint16_t *__restrict__ olist, const uint32_t *__restrict__ ocount,
+k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ lab16,
+            const unsigned long long *__restrict__ parent, const uint32_t *__restrict__ ocount,
             const uint8_t *__restrict__ in, uint8_t *__restrict__ out)
 {
     constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
-    __shared__ uint8_t s_dec[LAB_WORDS + NDEC];   // decision of the open cluster whose tile-local root is sp; constants
+    __shared__ uint8_t s_dec[OCAP + NDEC];   // [pos] decision of the tile's open root pos; [DEC_BASE + d] = d
 
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tid = threadIdx.x;
@@ -646,14 +701,12 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
     const uint32_t tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
     const uint32_t x0 = tx * TW, y0 = ty * TH;
 
-    // one decision per open root of the tile (S3; R5 CLUSTER stream), keyed on the global root K2b left
-    // in the open root's parent entry
+    pdl_prologue();
+    // one decision per open root of the tile (S3; R5 CLUSTER stream), keyed on the site index of the root
+    // of its cluster in the global union-find
     const uint32_t no = ocount[blockIdx.x];
-    uint32_t sp = 0u, r = 0u;
-    if (tid < no) {
-        sp = olist[(size_t)blockIdx.x * OCAP + tid];
-        r = (uint32_t)__ldg(parent + root_site(sp, x0, y0, L));
-    }
+    uint32_t r = 0u;
+    if (tid < no) r = groot_site(parent, blockIdx.x * (uint32_t)OCAP + tid);
     uint4 lab[PASSES];
 #pragma unroll
     for (int c = 0; c < PASSES; ++c) {
@@ -662,14 +715,11 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
     }
     if (tid < (uint32_t)NDEC) s_dec[DEC_BASE + tid] = (uint8_t)tid;
     for (uint32_t i = tid; i < no; i += TILE_THREADS) {
-        if (i >= TILE_THREADS) {
-            sp = olist[(size_t)blockIdx.x * OCAP + i];
-            r = (uint32_t)__ldg(parent + root_site(sp, x0, y0, L));
-        }
+        if (i >= TILE_THREADS) r = groot_site(parent, blockIdx.x * (uint32_t)OCAP + i);
         uint32_t w[4];
         philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
         const uint32_t ww = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
-        s_dec[sp] = (uint8_t)(MODEL == 0 ? mulhi_q(ww, (uint32_t)md.q) : (ww >> 31));
+        s_dec[i] = (uint8_t)(MODEL == 0 ? mulhi_q(ww, (uint32_t)md.q) : (ww >> 31));
     }
     __syncthreads();
 
@@ -683,7 +733,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
         const uint32_t w[4] = { lab[c].x, lab[c].y, lab[c].z, lab[c].w };
         uint32_t d[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) d[j] = s_dec[(w[j >> 1] >> (16 * (j & 1))) & LMASK];
+        for (int j = 0; j < 8; ++j) d[j] = s_dec[(w[j >> 1] >> (16 * (j & 1))) & 0x3FFu];   // LOPEN | pos or DEC_BASE + d
         uint2 o;
         if (MODEL == 0) {
             o.x = d[0] | (d[1] << 8) | (d[2] << 16) | (d[3] << 24);
@@ -708,7 +758,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
 }
 
 // Debug export (sw_get_labels): canonical root of every site.
-__global__ void k_resolve_labels(Model md, const uint16_t *__restrict__ lab16, const int32_t *__restrict__ parent,
+__global__ void k_resolve_labels(Model md, const uint16_t *__restrict__ lab16, const unsigned long long *__restrict__ parent,
                                  int32_t *__restrict__ out)
 {
     const uint32_t L = (uint32_t)md.L;
@@ -716,9 +766,9 @@ __global__ void k_resolve_labels(Model md, const uint16_t *__restrict__ lab16, c
     if (i >= md.N) return;
     const uint32_t y = i / L, x = i - y * L;
     const uint32_t v = lab16[i];
-    int32_t a = (int32_t)root_site(v, x - x % TW, y - y % TH, L);
-    if (v & LOPEN) a = uf_find(parent, a);
-    out[i] = a;
+    // written with fuse = 0: closed -> tile-local root sp; open -> LOPEN | pos
+    if (v & LOPEN) out[i] = (int32_t)groot_site(parent, ((y / TH) * (L / TW) + x / TW) * (uint32_t)OCAP + (v & (OCAP - 1u)));
+    else out[i] = (int32_t)root_site(v, x - x % TW, y - y % TH, L);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -736,31 +786,31 @@ static inline int tiled_init(TiledState &st, const Model &md, char *ws)
     st.vedge = reinterpret_cast<uint32_t *>(ws + off);
     off += ((L / TH) * (L / 32) * 4 + 1023) / 1024 * 1024;
     const size_t tiles = (L / TW) * (L / TH);
-    st.olist = reinterpret_cast<uint16_t *>(ws + off);
-    off += (tiles * OCAP * 2 + 1023) / 1024 * 1024;
+    st.edges = reinterpret_cast<uint16_t *>(ws + off);
+    off += (tiles * ECNT * 2 + 1023) / 1024 * 1024;
     st.ocount = reinterpret_cast<uint32_t *>(ws + off);
     return 0;
 }
 
-constexpr int TILED_NUM_KERNELS = 4;
-static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k_seam_merge", "k_open_flatten", "k_tile_flip" };
+constexpr int TILED_NUM_KERNELS = 3;
+static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k_seam_merge", "k_tile_flip" };
 
 static inline void tiled_launch_label(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
-                                      int32_t *parent, int fuse, cudaStream_t stream, unsigned long long *stats)
+                                      unsigned long long *parent, int fuse, cudaStream_t stream, unsigned long long *stats)
 {
     const uint32_t tiles = ((uint32_t)md.L / TW) * ((uint32_t)md.L / TH);
     if (md.model == 0)
-        k_tile_label<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.olist,
-                                                            st.ocount, fuse, stats);
+        launch_pdl(k_tile_label<0>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
+                   st.ocount, fuse, stats);
     else
-        k_tile_label<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.olist,
-                                                            st.ocount, fuse, stats);
+        launch_pdl(k_tile_label<1>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
+                   st.ocount, fuse, stats);
 }
 
 // One sweep: in = S^t (left untouched), out = S^{t+1}.  ev (optional): ev[0] is recorded before the first kernel,
 // ev[k+1] after kernel k.
 static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
-                              uint8_t *out, int32_t *parent, cudaStream_t stream, unsigned long long *stats,
+                              uint8_t *out, unsigned long long *parent, cudaStream_t stream, unsigned long long *stats,
                               uint64_t *launches, cudaEvent_t *ev)
 {
     const uint32_t L = (uint32_t)md.L;
@@ -769,28 +819,26 @@ static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &
     if (ev) cudaEventRecord(ev[0], stream);
     tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats);
     if (ev) cudaEventRecord(ev[1], stream);
-    k_seam_merge<<<(ne + 255) / 256, 256, 0, stream>>>(md, st.hedge, st.vedge, st.lab16, parent, stats);
+    launch_pdl(k_seam_merge, (ne + SW_SEAM_BS - 1) / SW_SEAM_BS, SW_SEAM_BS, stream, md, st.hedge, st.vedge, st.edges, parent, stats);
     if (ev) cudaEventRecord(ev[2], stream);
-    k_open_flatten<<<tiles, 128, 0, stream>>>(md, st.olist, st.ocount, parent);
-    if (ev) cudaEventRecord(ev[3], stream);
     if (md.model == 0)
-        k_tile_flip<0><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, st.lab16, parent, st.olist, st.ocount, in, out);
+        launch_pdl(k_tile_flip<0>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out);
     else
-        k_tile_flip<1><<<tiles, TILE_THREADS, 0, stream>>>(md, key, t, st.lab16, parent, st.olist, st.ocount, in, out);
-    if (ev) cudaEventRecord(ev[4], stream);
-    *launches += 4;
+        launch_pdl(k_tile_flip<1>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out);
+    if (ev) cudaEventRecord(ev[3], stream);
+    *launches += 3;
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
 }
 
 // Debug export (sw_get_labels): label the configuration `in` with the bonds of sweep t again, this time keeping the
 // tile-local root of every site (no fused decisions), merge, and resolve every site to its canonical root.
 static inline int tiled_relabel(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
-                                int32_t *parent, int32_t *out, cudaStream_t stream, uint64_t *launches)
+                                unsigned long long *parent, int32_t *out, cudaStream_t stream, uint64_t *launches)
 {
     const uint32_t L = (uint32_t)md.L;
     const uint32_t ne = (L / TW) * L + (L / TH) * L;
     tiled_launch_label(st, md, key, t, in, parent, 0, stream, nullptr);
-    k_seam_merge<<<(ne + 255) / 256, 256, 0, stream>>>(md, st.hedge, st.vedge, st.lab16, parent, nullptr);
+    launch_pdl(k_seam_merge, (ne + SW_SEAM_BS - 1) / SW_SEAM_BS, SW_SEAM_BS, stream, md, st.hedge, st.vedge, st.edges, parent, (unsigned long long *)nullptr);
     k_resolve_labels<<<(md.N + 255) / 256, 256, 0, stream>>>(md, st.lab16, parent, out);
     *launches += 3;
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
