@@ -43,7 +43,7 @@ constexpr uint32_t LOPEN = 0x8000u;     // cluster may continue in another tile
 constexpr int LAB_WORDS = TILE_SITES + TILE_SITES / 32;   // skewed tile-local index sp = p + (p >> 5)
 constexpr int EDGE_CAP = 256;           // union edges listed per warp (more are handled by their own thread)
 constexpr int NDEC = 16;               // decisions are < q <= 16
-constexpr int RCAP = 256;               // closed roots listed per warp for the converged decision draw
+constexpr int RCAP = 512;               // closed roots listed per warp for the converged decision draw
 constexpr int DEC_BASE = 512;           // lab16 value DEC_BASE + d: "closed cluster, decision d" (= OCAP)
 constexpr int ECNT = 2 * TH + 2 * TW;     // edge labels exported per tile: left column, right column, top row, bottom row
 constexpr int OCAP = 512;               // open roots listed per tile (<= 128 + 64 + 128 + 64 boundary positions)
@@ -260,7 +260,10 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     const uint32_t g = u & hin, sum = hin + g;
     const uint32_t first = (g & (sum ^ hin)) | (u & ~hin & ~sum);
     // up-bonds that still need a union: not the first of their run, and not parallel to the bond on their left
-    const uint32_t X = u & ~first & ~((u & ha & hin) << 1);
+    // (an up-bond is redundant if a lower up-bond of the same run reaches the same run above: both rows linked all the
+    // way between them -- the carry-in mask of C + (u & C), C = links present in both rows)
+    const uint32_t C = ha & hin, gC = u & C;
+    const uint32_t X = u & ~first & ~((C + gC) ^ C ^ gC);
     const bool hedge_out = (ww + 1u < (uint32_t)NWORD) && (h >> 31);
     uint32_t epos;                                            // this thread's first slot in the warp's edge list
     uint32_t etotal;
@@ -461,7 +464,16 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
             const uint32_t v = vl[sb + k];
             if ((v & LMASK) == sb + k) {
-                if (v & LOPEN) rooto |= 1u << k; else rootc |= 1u << k;
+                bool on_axis = false;
+                if (MODEL == 1) {
+                    // a spin on the mirror axis has no active bond at all (its thresholds are 0, R4) and the
+                    // reflection maps it to itself: a closed singleton whose decision is never used -- no draw
+                    const uint32_t c = clock_c(spins[(size_t)(y0 + wy) * L + x0 + ww * 32u + k], m, q2);
+                    on_axis = (c == 0u) || (c == (uint32_t)md.q);
+                }
+                if (on_axis) vl[sb + k] = (sb + k) | ((fuse ? (uint32_t)DEC_BASE : sb + k) << 16);
+                else if (v & LOPEN) rooto |= 1u << k;
+                else rootc |= 1u << k;
             }
         }
         // compact the warp's roots into its list (reusing the second half of the warp's edge list), so that the
