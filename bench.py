@@ -28,7 +28,7 @@ if str(ROOT) not in sys.path:
 METRIC = "ns per spin flip (full SW sweep) at L=4096, T_c"
 UNIT = "ns/spin-flip"
 B_ALG = 10.0            # algorithmic HBM bytes per spin per sweep: 1+4 (label) + 4+1 (flip)
-B_ALG_KERNEL = {"k_tile_label": 5.0, "k_flip_tiled": 5.0, "k_flip": 5.0}   # per spin, per launch
+B_ALG_KERNEL = {"k_tile_label": 5.0, "k_tile_flip": 5.0, "k_flip": 5.0}   # per spin, per launch
 
 
 def peaks():
@@ -167,7 +167,8 @@ def main():
 
     w = CONFIGS[args.workload or HEADLINE]
     L, q, N = w.L, w.q, w.L * w.L
-    seed = w.seed + 7919 * rank                       # replicas only: every rank its own lattice
+    from paper_1202_0635_b200 import replicas
+    seed = replicas.replica_seed(w.seed, rank)       # replicas only: every rank its own lattice
     lat = sw.Lattice(L, q, w.model, w.T, seed)
     stream = torch.cuda.current_stream()
     l2_flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
@@ -250,16 +251,10 @@ def main():
         host_in, host_out = host_out, host_in
     barrier()
     e2e_s = time.perf_counter() - t0
-    t_e2e = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    t_dev = torch.tensor([total_ms, b2b_ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
-        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-    total_ms, b2b_ms = float(t_dev[0]), float(t_dev[1])
-    e2e_s = float(t_e2e[0])
+    total_ms, b2b_ms, e2e_s = replicas.max_over_ranks([total_ms, b2b_ms, e2e_s], dist, device="cuda")
 
     flips = float(world) * args.steps * N
-    value = total_ms * 1e6 / flips                    # ns per spin flip, whole job
+    value = replicas.whole_job_ns_per_flip(total_ms, args.steps, N, world)   # ns per spin flip, whole job
     e2e_value = e2e_s * 1e9 / (float(world) * e2e_steps * N)
 
     cpu = None

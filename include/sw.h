@@ -109,8 +109,8 @@ int sw_get_algorithm(sw_ctx *ctx); /* the back-end actually in use (never SW_ALG
  * PAPER.md:75), HOST output of SW_NUM_STATS doubles: out[0] = sweeps counted, out[1] = cross-tile merge attempts,
  * out[2] = tile-local nodes (horizontal runs), out[3] = tile-local union edges, out[4] = pointer hops of the
  * tile-local resolve pass, out[5..7] reserved (0), out[8..15] = SM clock cycles the warps of the tile-labeling
- * kernel spent in each of its phases (bonds, setup, run scan, unions, open marking, resolve, output; summed over
- * warps).  Counters are only collected after sw_enable_stats(ctx, 1) (they cost atomics and clock reads). */
+ * kernel spent in each of its phases (bonds, setup, run scan, unions, open marking, resolve, output, root decisions;
+ * summed over warps).  Counters are only collected after sw_enable_stats(ctx, 1) (they cost atomics and clock reads). */
 #define SW_NUM_STATS 16
 int sw_enable_stats(sw_ctx *ctx, int on);
 int sw_stats(sw_ctx *ctx, double *out);

@@ -1,27 +1,28 @@
-// Tiled back-end (SW_ALGO_TILED), L % 128 == 0.  One sweep = three kernels:
+// Tiled back-end (SW_ALGO_TILED), L % 128 == 0.  One sweep = three kernels, chained by programmatic dependent launch:
 //
-//   K1 k_tile_label   S1 + S2a.  One CTA owns a 128 x 64 tile.
-//        phase A  bonds: Philox in registers (one call per two sites), compared with the integer threshold;
-//                 the 2 bits per site are packed into row bit masks H (bond to +x) and V (bond to +y) in
-//                 shared memory.  Bonds never go to HBM; only the bits that cross a tile edge are exported.
+//   K1 k_tile_label   S1 + S2a + S3 for the clusters that end inside a tile.  One CTA owns a 128 x 64 tile.
+//        phase A  bonds: Philox in registers (one call per two sites), compared with the integer threshold; the
+//                 2 bits per site are packed into row bit masks H (bond to +x) and V (bond to +y) in shared memory.
+//                 Bonds never go to HBM; only the bits that cross a tile edge are exported (hedge / vedge).
 //        phase B  labeling on the masks, one thread per 32-site word.  A node = a horizontal run clipped to its
-//                 word, named by the tile-local index of its first site, so all +x bonds inside a word are
-//                 merged by bit arithmetic alone.  Every node with a bond to the row above inherits (plain
-//                 store) the node above its lowest such bond; only the remaining, non-redundant up-bonds and
-//                 the bonds between words go through the shared-memory union-find (atomicMin, root = smallest
-//                 index: the "proper label ... smallest" of PAPER.md:47 at tile level).
-//        output   one uint16 per site: the tile-local index of the tile-local root, bit 15 = the cluster may
-//                 continue in another tile ("open").  Open roots also initialise their entry of the global
-//                 parent array.
-//   K2 k_seam_merge   S2b: union (global atomicMin union-find on `parent`, indexed by site) across every active
-//                     tile-crossing bond.  Touches tile-edge sites and open roots only.
-//   K3 k_tile_flip    S3 + S4.  Per tile: compact the tile-local roots, resolve the open ones to their global
-//                     root (short chase), draw the cluster decision from the CLUSTER stream keyed on that root
-//                     -- once per root, not once per site (the paper draws one per label number) --
-//                     then every site looks its root's decision up in shared memory and updates its spin.
+//                 word, named by the tile-local index of its first site, so all +x bonds inside a word are merged by
+//                 bit arithmetic alone.  B1: every run with a bond to the row above inherits (plain store) the run
+//                 above its lowest such bond; B2: only the remaining, non-redundant up-bonds and the bonds between
+//                 words go through the shared-memory union-find (atomicMin, root = smallest index: the "proper
+//                 label ... smallest" of PAPER.md:47 at tile level); B3: clusters that may continue in another
+//                 tile are marked open; B3b: every closed root draws its cluster's decision (CLUSTER stream keyed
+//                 on its global site index), every open root becomes node tile * OCAP + pos of the global
+//                 union-find; B4: every run resolves to its root.
+//        output   one uint16 per site: DEC_BASE + decision (closed cluster) or LOPEN | pos (open cluster); the labels
+//                 of the tile's boundary sites also go to a compact edge array for K2.
+//   K2 k_seam_merge   S2b: union across every active tile-crossing bond in the global union-find over open roots
+//                     (64-bit keys (site index, node), atomicMin: the root of a cluster is its minimum site index).
+//   K3 k_tile_flip    S3 for open clusters + S4.  Per tile: one decision per open root, keyed on the site index of its
+//                     global root; then every site looks its 16-bit label up in a 528-byte table and the new spin is
+//                     written to the other ping-pong buffer.
 //
-// The root of a cluster is its minimum site index at both levels (row-major order inside a tile equals the
-// order of the global indices), so spins, labels and observables equal the oracle's bit for bit.
+// The root of a cluster is its minimum site index at both levels (row-major order inside a tile equals the order
+// of the global indices), so spins, labels and observables equal the oracle's bit for bit.
 // HBM traffic per site and sweep: K1 1 B (spins) + 2 B (labels); K3 2 B (labels) [+ 1 B spins, clock] + 1 B.
 #pragma once
 #include <cuda_runtime.h>
@@ -315,6 +316,12 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     }
     __syncthreads();
     SW_PHASE(2)
+#ifndef SW_B2_DYN
+#define SW_B2_DYN 1
+#endif
+#ifndef SW_RESOLVE_PASSES
+#define SW_RESOLVE_PASSES 2
+#endif
 #ifndef SW_RESOLVE_CHUNK
 #define SW_RESOLVE_CHUNK 4
 #endif
@@ -359,6 +366,37 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         // Every lane keeps SW_B2_ILP edges in flight: the pointer loads of the edges are independent, so their
         // shared-memory latencies overlap; a lane leaves the loop when all its edges of the batch are merged.
         volatile uint32_t *vl = s_lab;
+#if SW_B2_DYN
+        // One edge in flight per lane; a lane that has merged its edge takes the next unclaimed one of the warp's
+        // list at once (shared counter), so no lane waits for the slowest edge of a batch.
+        {
+            uint32_t e = lane, ea = 0u, eb = 0u;
+            bool have = e < ne;
+            if (have) { const uint32_t v = s_edge[warp][e]; ea = v & 0xFFFFu; eb = v >> 16; }
+            while (have) {
+                const uint32_t pa = vl[ea], pb = vl[eb];
+                const uint32_t ga = vl[pa], gb = vl[pb];
+                bool done = false;
+                if (pa != ea || pb != eb) {
+                    if (ga != pa) vl[ea] = ga;                   // path halving: skip one ancestor on each side
+                    if (gb != pb) vl[eb] = gb;
+                    ea = ga; eb = gb;
+                } else if (ea == eb) {
+                    done = true;
+                } else {
+                    const uint32_t hi = ea > eb ? ea : eb, lo = ea > eb ? eb : ea;
+                    const uint32_t old = atomicMin(s_lab + hi, lo);
+                    if (old == hi) done = true;
+                    else { ea = old; eb = lo; }                  // hi had a parent already: keep it connected to lo
+                }
+                if (done) {
+                    e = atomicAdd(&s_enext[warp], 1u);
+                    have = e < ne;
+                    if (have) { const uint32_t v = s_edge[warp][e]; ea = v & 0xFFFFu; eb = v >> 16; }
+                }
+            }
+        }
+#else
         for (uint32_t e0 = lane; e0 < ne; e0 += 32u * SW_B2_ILP) {
             uint32_t a[SW_B2_ILP], b[SW_B2_ILP];
             uint32_t live = 0u;
@@ -403,6 +441,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
                 }
             }
         }
+#endif
         if (etotal > (uint32_t)EDGE_CAP && epos > (uint32_t)EDGE_CAP) {
             // rare: the list overflowed; this thread unions its unlisted edges itself
             uint32_t slot = epos0, Xr = X;
@@ -538,27 +577,33 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     uint32_t hops = 0u;
     {
         volatile uint32_t *vl = s_lab;
-        uint32_t rem = 0u;
-        uint32_t sr = S;
-        while (sr) {
-            uint32_t kk[4], x[4], y[4];
+        // one pass over the runs in `todo`: returns the runs that are still not at their root
+        auto pass = [&](uint32_t todo) -> uint32_t {
+            uint32_t rem = 0u;
+            while (todo) {
+                uint32_t kk[4], x[4], y[4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                kk[j] = sr ? (uint32_t)__ffs((int)sr) - 1u : kk[0];
-                sr &= sr - 1u;
+                for (int j = 0; j < 4; ++j) {
+                    kk[j] = todo ? (uint32_t)__ffs((int)todo) - 1u : kk[0];
+                    todo &= todo - 1u;
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) x[j] = vl[sb + kk[j]];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) x[j] = vl[x[j] & LMASK];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) y[j] = vl[x[j] & LMASK];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    vl[sb + kk[j]] = y[j];
+                    if ((y[j] ^ x[j]) & LMASK) rem |= 1u << kk[j];
+                }
             }
-#pragma unroll
-            for (int j = 0; j < 4; ++j) x[j] = vl[sb + kk[j]];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) x[j] = vl[x[j] & LMASK];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) y[j] = vl[x[j] & LMASK];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                vl[sb + kk[j]] = y[j];
-                if ((y[j] ^ x[j]) & LMASK) rem |= 1u << kk[j];
-            }
-        }
+            return rem;
+        };
+        uint32_t rem = pass(S);
+#pragma unroll 1
+        for (int r = 0; r < SW_RESOLVE_PASSES - 1; ++r) rem = pass(rem);   // the written-back pointers of all runs shorten these
         while (rem) {
             const uint32_t k = 31u - (uint32_t)__clz((int)rem);
             rem ^= 1u << k;
