@@ -225,11 +225,18 @@ def main():
     peak, peak_src = peaks()
     dom_bytes = B_ALG_KERNEL.get(dom, 5.0) * N
     achieved = dom_bytes / (prof[dom] * 1e-3) / 1e9
-    traffic = None
+    traffic, issue = None, None
     tr = ROOT / "profiles" / "traffic.json"
-    if tr.exists():
+    if tr.exists() and w.name == HEADLINE:
         try:
-            traffic = json.loads(tr.read_text()).get(dom)
+            tj = json.loads(tr.read_text())
+            traffic = tj.get(dom)
+            winst = tj.get(dom + "_warp_instructions")
+            if winst:
+                # the co-limit DESIGN.md section 6 names: warp-instruction issue slots, 148 SMs x 4 schedulers x SM clock
+                ipeak = 148 * 4 * (clocks["sm_mhz"] or 1965.0) * 1e6
+                issue = {"bound": "alu", "achieved": winst / (prof[dom] * 1e-3), "peak": ipeak, "unit": "warp-instr/s",
+                         "frac": winst / (prof[dom] * 1e-3) / ipeak, "source": "ncu smsp__inst_executed.sum (profiles/r1_final.md) / live kernel time"}
         except Exception:
             traffic = None
 
@@ -282,6 +289,7 @@ def main():
                          "traffic": traffic, "peak_source": peak_src, "ms_per_launch": prof[dom],
                          "algorithmic_bytes_per_launch": dom_bytes},
             "sweep_roofline": {"bytes_per_spin": B_ALG, "achieved_gbs": sweep_gbs, "frac": sweep_gbs / peak},
+            "issue_roofline": issue,
             "kernels_ms": prof,
             "cpu_baseline": cpu,
             "paper_context": {"gtx580_ns_per_spin_flip": 2.51, "source": "PAPER.md:83 Table 1 (another machine: context, not the target)"},
