@@ -12,12 +12,14 @@ stream sees the kernels.
 from __future__ import annotations
 
 import ctypes
+import os
 from pathlib import Path
 
 import numpy as np
 
 _PKG = Path(__file__).resolve().parent
-LIB_PATH = _PKG / "libsw.so"
+# SW_LIB: load another build of the same library (tests/test_gpu_parity.py builds one with tiny list capacities)
+LIB_PATH = Path(os.environ["SW_LIB"]) if os.environ.get("SW_LIB") else _PKG / "libsw.so"
 
 SW_POTTS, SW_CLOCK = 0, 1
 SW_OK, SW_ERR_ARG, SW_ERR_CUDA, SW_ERR_NOMEM, SW_ERR_UNSUPPORTED = 0, -1, -2, -3, -4

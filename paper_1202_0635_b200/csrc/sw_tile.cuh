@@ -42,9 +42,15 @@ constexpr int ROWS_PER_WARP = 8;        // TILE_THREADS / 32 warps x 8 rows = TH
 constexpr uint32_t LMASK = 0x3FFFu;     // local index field of a label
 constexpr uint32_t LOPEN = 0x8000u;     // cluster may continue in another tile
 constexpr int LAB_WORDS = TILE_SITES + TILE_SITES / 32;   // skewed tile-local index sp = p + (p >> 5)
-constexpr int EDGE_CAP = 256;           // union edges listed per warp (more are handled by their own thread)
+#ifndef SW_EDGE_CAP
+#define SW_EDGE_CAP 256   // tests build a variant with tiny lists to drive the overflow paths
+#endif
+#ifndef SW_RCAP
+#define SW_RCAP 512
+#endif
+constexpr int EDGE_CAP = SW_EDGE_CAP;           // union edges listed per warp (more are handled by their own thread)
 constexpr int NDEC = 16;               // decisions are < q <= 16
-constexpr int RCAP = 512;               // closed roots listed per warp for the converged decision draw
+constexpr int RCAP = SW_RCAP;               // closed roots listed per warp for the converged decision draw
 constexpr int DEC_BASE = 512;           // lab16 value DEC_BASE + d: "closed cluster, decision d" (= OCAP)
 constexpr int ECNT = 2 * TH + 2 * TW;     // edge labels exported per tile: left column, right column, top row, bottom row
 constexpr int OCAP = 512;               // open roots listed per tile (<= 128 + 64 + 128 + 64 boundary positions)
@@ -316,26 +322,11 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     }
     __syncthreads();
     SW_PHASE(2)
-#ifndef SW_B2_DYN
-#define SW_B2_DYN 1
-#endif
 #ifndef SW_RESOLVE_PASSES
 #define SW_RESOLVE_PASSES 2
 #endif
-#ifndef SW_RESOLVE_CHUNK
-#define SW_RESOLVE_CHUNK 4
-#endif
-#ifndef SW_B2_ILP
-#define SW_B2_ILP 1
-#endif
-#ifndef SW_B2_HALVE
-#define SW_B2_HALVE 1
-#endif
 #ifndef SW_JUMP_ROUNDS
 #define SW_JUMP_ROUNDS 0
-#endif
-#ifndef SW_B4_WRITEBACK
-#define SW_B4_WRITEBACK 1
 #endif
     // B1b: pointer jumping on the inheritance forest (plain stores only so far: any ancestor is a valid parent, so the
     // rounds need no barrier between them).  Shallow trees make the finds of B2 and the resolve pass of B4a short.
@@ -363,10 +354,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     // B2: the warp's edges, one per lane and round (union-find by minimum index: PAPER.md:47 at tile level)
     {
         const uint32_t ne = etotal < (uint32_t)EDGE_CAP ? etotal : (uint32_t)EDGE_CAP;
-        // Every lane keeps SW_B2_ILP edges in flight: the pointer loads of the edges are independent, so their
-        // shared-memory latencies overlap; a lane leaves the loop when all its edges of the batch are merged.
         volatile uint32_t *vl = s_lab;
-#if SW_B2_DYN
         // One edge in flight per lane; a lane that has merged its edge takes the next unclaimed one of the warp's
         // list at once (shared counter), so no lane waits for the slowest edge of a batch.
         {
@@ -396,52 +384,6 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
                 }
             }
         }
-#else
-        for (uint32_t e0 = lane; e0 < ne; e0 += 32u * SW_B2_ILP) {
-            uint32_t a[SW_B2_ILP], b[SW_B2_ILP];
-            uint32_t live = 0u;
-#pragma unroll
-            for (int j = 0; j < SW_B2_ILP; ++j) {
-                const uint32_t e = e0 + 32u * j;
-                a[j] = b[j] = 0u;
-                if (e < ne) {
-                    const uint32_t v = s_edge[warp][e];
-                    a[j] = v & 0xFFFFu; b[j] = v >> 16;
-                    live |= 1u << j;
-                }
-            }
-            while (live) {
-                uint32_t pa[SW_B2_ILP], pb[SW_B2_ILP];
-#pragma unroll
-                for (int j = 0; j < SW_B2_ILP; ++j) { pa[j] = vl[a[j]]; pb[j] = vl[b[j]]; }
-#if SW_B2_HALVE
-                uint32_t ga[SW_B2_ILP], gb[SW_B2_ILP];
-#pragma unroll
-                for (int j = 0; j < SW_B2_ILP; ++j) { ga[j] = vl[pa[j]]; gb[j] = vl[pb[j]]; }
-#endif
-#pragma unroll
-                for (int j = 0; j < SW_B2_ILP; ++j) {
-                    if (!((live >> j) & 1u)) continue;
-                    if (pa[j] != a[j] || pb[j] != b[j]) {
-#if SW_B2_HALVE
-                        if (ga[j] != pa[j]) vl[a[j]] = ga[j];     // path halving: skip one ancestor on each side
-                        if (gb[j] != pb[j]) vl[b[j]] = gb[j];
-                        a[j] = ga[j]; b[j] = gb[j];
-#else
-                        a[j] = pa[j]; b[j] = pb[j];
-#endif
-                    } else if (a[j] == b[j]) {
-                        live &= ~(1u << j);
-                    } else {
-                        const uint32_t hi = a[j] > b[j] ? a[j] : b[j], lo = a[j] > b[j] ? b[j] : a[j];
-                        const uint32_t old = atomicMin(s_lab + hi, lo);
-                        if (old == hi) live &= ~(1u << j);
-                        else { a[j] = old; b[j] = lo; }           // hi had a parent already: keep it connected to lo
-                    }
-                }
-            }
-        }
-#endif
         if (etotal > (uint32_t)EDGE_CAP && epos > (uint32_t)EDGE_CAP) {
             // rare: the list overflowed; this thread unions its unlisted edges itself
             uint32_t slot = epos0, Xr = X;
@@ -660,21 +602,14 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
 // decrease, so a stale read is still an ancestor and the atomicMin re-validates the root.
 __device__ __forceinline__ unsigned long long gfind(unsigned long long *parent, uint32_t x)
 {
-#ifndef SW_SEAM_EXP
-#define SW_SEAM_EXP 0
-#endif
-#if SW_SEAM_EXP == 3
-#define GLD(p_) __ldcg(p_)
-#else
-#define GLD(p_) (*(p_))
-#endif
-    unsigned long long p = GLD(parent + x);
+    // plain (L1-cacheable) loads: a stale line still holds an ancestor, and hot roots stay out of L2
+    unsigned long long p = parent[x];
     uint32_t prev = x;
     while ((uint32_t)p != prev) {
         const uint32_t cur = (uint32_t)p;
-        const unsigned long long g = GLD(parent + cur);
+        const unsigned long long g = parent[cur];
         if ((uint32_t)g == cur) return g;
-        if (SW_SEAM_EXP != 2) parent[prev] = g;                     // path halving
+        parent[prev] = g;                     // path halving
         prev = cur;
         p = g;
     }
@@ -705,10 +640,8 @@ __device__ __forceinline__ uint32_t groot_site(const unsigned long long *__restr
 // K2.  One thread per tile-edge bond position: first the (L/128)*L right-edge bonds, then the (L/TH)*L bottom-edge
 // bonds.  The two ends of an active tile-crossing bond lie in open clusters; their lab16 values (LOPEN | pos) come
 // from the compact edge arrays K1 wrote.
-#ifndef SW_SEAM_BS
-#define SW_SEAM_BS 256
-#endif
-__global__ void __launch_bounds__(SW_SEAM_BS)
+constexpr int SEAM_THREADS = 256;
+__global__ void __launch_bounds__(SEAM_THREADS)
 k_seam_merge(Model md, const uint32_t *__restrict__ hedge, const uint32_t *__restrict__ vedge,
              const uint16_t *__restrict__ edges, unsigned long long *parent, unsigned long long *stats)
 {
@@ -738,7 +671,6 @@ k_seam_merge(Model md, const uint32_t *__restrict__ hedge, const uint32_t *__res
     const uint32_t a = edges[(size_t)ta * ECNT + ia], b = edges[(size_t)tb * ECNT + ib];
     if (!bit) return;
     if (stats) atomicAdd(stats + 1, 1ull);
-    if (SW_SEAM_EXP == 1) { if (a == 0xFFFFu && b == 0xFFFEu) parent[0] = 0; return; }
     gunion(parent, ta * OCAP + (a & (OCAP - 1u)), tb * OCAP + (b & (OCAP - 1u)));
 }
 
@@ -876,7 +808,7 @@ static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &
     if (ev) cudaEventRecord(ev[0], stream);
     tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats);
     if (ev) cudaEventRecord(ev[1], stream);
-    launch_pdl(k_seam_merge, (ne + SW_SEAM_BS - 1) / SW_SEAM_BS, SW_SEAM_BS, stream, md, st.hedge, st.vedge, st.edges, parent, stats);
+    launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent, stats);
     if (ev) cudaEventRecord(ev[2], stream);
     if (md.model == 0)
         launch_pdl(k_tile_flip<0>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out);
@@ -895,7 +827,7 @@ static inline int tiled_relabel(TiledState &st, const Model &md, const PhiloxKey
     const uint32_t L = (uint32_t)md.L;
     const uint32_t ne = (L / TW) * L + (L / TH) * L;
     tiled_launch_label(st, md, key, t, in, parent, 0, stream, nullptr);
-    launch_pdl(k_seam_merge, (ne + SW_SEAM_BS - 1) / SW_SEAM_BS, SW_SEAM_BS, stream, md, st.hedge, st.vedge, st.edges, parent, (unsigned long long *)nullptr);
+    launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent, (unsigned long long *)nullptr);
     k_resolve_labels<<<(md.N + 255) / 256, 256, 0, stream>>>(md, st.lab16, parent, out);
     *launches += 3;
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
