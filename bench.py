@@ -231,12 +231,14 @@ def main():
         try:
             tj = json.loads(tr.read_text())
             traffic = tj.get(dom)
-            winst = tj.get(dom + "_warp_instructions")
-            if winst:
-                # the co-limit DESIGN.md section 6 names: warp-instruction issue slots, 148 SMs x 4 schedulers x SM clock
+            winst, dcyc = tj.get(dom + "_warp_instructions"), tj.get(dom + "_dispatch_cycles")
+            if winst and dcyc:
+                # the bound DESIGN.md sections 6 and 11 derive: math-dispatch cycles, 148 SMs x 4 schedulers x SM clock
+                # (an ALU-pipe or IMAD.WIDE warp instruction takes two dispatch cycles, a 32-bit IMAD one)
                 ipeak = 148 * 4 * (clocks["sm_mhz"] or 1965.0) * 1e6
-                issue = {"bound": "alu", "achieved": winst / (prof[dom] * 1e-3), "peak": ipeak, "unit": "warp-instr/s",
-                         "frac": winst / (prof[dom] * 1e-3) / ipeak, "source": "ncu smsp__inst_executed.sum (profiles/r1_final.md) / live kernel time"}
+                issue = {"bound": "alu", "achieved": dcyc / (prof[dom] * 1e-3), "peak": ipeak, "unit": "dispatch-cycles/s",
+                         "frac": dcyc / (prof[dom] * 1e-3) / ipeak, "warp_instructions_per_launch": winst,
+                         "source": "executed-opcode histogram of the committed ncu capture (profiles/r1_final.md) / live kernel time"}
         except Exception:
             traffic = None
 
