@@ -512,7 +512,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     if (tid == 0u) ocount[blockIdx.x] = s_nopen;
 
     SW_PHASE(7)
-    // B4a: resolve every run of the word to its root's entry (whose upper half is the output value).  Four runs at
+    // B4a: resolve every run of the word to its root's entry (whose upper half is the output value).  Two runs at
     // a time, three pointer hops each (the loads of one level are independent, so their latencies overlap), result
     // written back to the run's own entry; runs deeper than that (rare) are finished by a chase that starts from the
     // already advanced pointer.
@@ -523,23 +523,17 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         auto pass = [&](uint32_t todo) -> uint32_t {
             uint32_t rem = 0u;
             while (todo) {
-                uint32_t kk[4], x[4], y[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    kk[j] = todo ? (uint32_t)__ffs((int)todo) - 1u : kk[0];
-                    todo &= todo - 1u;
-                }
-#pragma unroll
-                for (int j = 0; j < 4; ++j) x[j] = vl[sb + kk[j]];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) x[j] = vl[x[j] & LMASK];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) y[j] = vl[x[j] & LMASK];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    vl[sb + kk[j]] = y[j];
-                    if ((y[j] ^ x[j]) & LMASK) rem |= 1u << kk[j];
-                }
+                // the lowest and the highest run still to do (the same run when one is left: harmless repeat)
+                const uint32_t k0 = (uint32_t)__ffs((int)todo) - 1u, k1 = 31u - (uint32_t)__clz((int)todo);
+                todo &= todo - 1u;
+                todo &= ~(1u << k1);
+                uint32_t x0 = vl[sb + k0], x1 = vl[sb + k1];
+                x0 = vl[x0 & LMASK]; x1 = vl[x1 & LMASK];
+                const uint32_t y0r = vl[x0 & LMASK], y1r = vl[x1 & LMASK];
+                vl[sb + k0] = y0r;
+                vl[sb + k1] = y1r;
+                if ((y0r ^ x0) & LMASK) rem |= 1u << k0;
+                if ((y1r ^ x1) & LMASK) rem |= 1u << k1;
             }
             return rem;
         };
