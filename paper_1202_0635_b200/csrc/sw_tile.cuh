@@ -440,7 +440,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     // the CLUSTER stream keyed on the root's global site index (R5).
     {
         volatile uint32_t *vl = s_lab;
-        uint32_t rootc = 0u, rooto = 0u;
+        uint32_t rall = 0u;                       // this word's roots (their entries: sp, or sp | LOPEN when open)
         for (uint32_t c = cs; c; c &= c - 1u) {
             const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
             const uint32_t v = vl[sb + k];
@@ -453,14 +453,12 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
                     on_axis = (c == 0u) || (c == (uint32_t)md.q);
                 }
                 if (on_axis) vl[sb + k] = (sb + k) | ((fuse ? (uint32_t)DEC_BASE : sb + k) << 16);
-                else if (v & LOPEN) rooto |= 1u << k;
-                else rootc |= 1u << k;
+                else rall |= 1u << k;
             }
         }
         // compact the warp's roots into its list (reusing the second half of the warp's edge list), so that the
         // decisions are drawn -- and the open roots registered -- with all lanes busy
         uint16_t *rl = reinterpret_cast<uint16_t *>(&s_edge[warp][0]) + 2 * (EDGE_CAP + 1) - RCAP;
-        const uint32_t rall = rootc | rooto;
         const uint32_t n = __popc(rall);
         uint32_t incl = n;
 #pragma unroll
@@ -474,7 +472,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             uint32_t at = incl - n;
             for (uint32_t rr = rall; rr; rr &= rr - 1u) {
                 const uint32_t k = (uint32_t)__ffs((int)rr) - 1u;
-                rl[at++] = (uint16_t)((sb + k) | (((rooto >> k) & 1u) ? LOPEN : 0u));
+                rl[at++] = (uint16_t)vl[sb + k];
             }
             __syncwarp();
         }
@@ -488,7 +486,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             } else {
                 const uint32_t k = (uint32_t)__ffs((int)mine) - 1u;
                 mine &= mine - 1u;
-                e = (sb + k) | (((rooto >> k) & 1u) ? LOPEN : 0u);
+                e = vl[sb + k] & 0xFFFFu;
             }
             const uint32_t sp = e & LMASK;
             const uint32_t r = root_site(sp, x0, y0, L);
