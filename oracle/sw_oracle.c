@@ -281,6 +281,23 @@ void oracle_observables(int L, int q, const uint8_t *spins, int64_t *bond_hist, 
     }
 }
 
+/* Correlation histogram at distance r (eq.(5), eq.(6); R15):   */
+/* corr_hist[d] = number of pairs (i, i + r e_x) and (i, i + r e_y), periodic, with (S_i - S_{i+r}) mod q  */
+/* == d; 2N pairs.  G(r) = (1/2N) sum_d corr_hist[d] cos(2 pi d / q) is derived by the caller.             */
+void oracle_correlation(int L, int q, const uint8_t *spins, int r, int64_t *corr_hist)
+{
+    for (int k = 0; k < q; ++k) corr_hist[k] = 0;
+    for (int y = 0; y < L; ++y) {
+        for (int x = 0; x < L; ++x) {
+            int s = spins[y * L + x];
+            int sx = spins[y * L + (x + r) % L];
+            int sy = spins[((y + r) % L) * L + x];
+            corr_hist[((s - sx) % q + q) % q] += 1;
+            corr_hist[((s - sy) % q + q) % q] += 1;
+        }
+    }
+}
+
 /* n sweeps t0 .. t0+n-1.  If bond_rec/state_rec are non-NULL, row k (q entries each) receives
  * the observables of the configuration BEFORE sweep t0+k (R10). */
 int oracle_run(int L, int q, int model, double T, uint64_t seed, uint32_t t0, int n,

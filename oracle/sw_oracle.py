@@ -73,6 +73,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_sweep.restype = ctypes.c_int
         L.oracle_observables.argtypes = [ctypes.c_int, ctypes.c_int, _u8p, _i64p, _i64p]
         L.oracle_observables.restype = None
+        L.oracle_correlation.argtypes = [ctypes.c_int, ctypes.c_int, _u8p, ctypes.c_int, _i64p]
+        L.oracle_correlation.restype = None
         L.oracle_run.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                  ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int, _u8p, _i64p, _i64p]
         L.oracle_run.restype = ctypes.c_int
@@ -165,6 +167,14 @@ def observables(L, q, spins):
     sh = np.zeros(q, dtype=np.int64)
     lib().oracle_observables(L, q, _p(s, _u8p), _p(bh, _i64p), _p(sh, _i64p))
     return bh, sh
+
+
+def correlation(L, q, spins, r):
+    """corr_hist[d] = #{pairs at distance r along +x and +y with (S_i - S_j) mod q == d} (eq.(5); R15)."""
+    s = np.ascontiguousarray(spins, dtype=np.uint8).reshape(L, L)
+    ch = np.zeros(q, dtype=np.int64)
+    lib().oracle_correlation(L, q, _p(s, _u8p), int(r), _p(ch, _i64p))
+    return ch
 
 
 def run(L, q, model, T, seed, t0, n, spins, record=False):
