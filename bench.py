@@ -211,6 +211,14 @@ def main():
     e1.record(stream)
     barrier()
     b2b_ms = e0.elapsed_time(e1)
+    # the paper's second column: update + measurement of energy and magnetisation every sweep
+    barrier()
+    m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    m0.record(stream)
+    lat.sweep_record(args.steps)
+    m1.record(stream)
+    barrier()
+    meas_ms = m0.elapsed_time(m1)
     clocks = sampler.stop()
 
     # ---- per-kernel device time (events between kernels), L2 flushed before each sweep ----------------------
@@ -284,6 +292,8 @@ def main():
                        "parallelism": "replicas only" if world > 1 else "single GPU", "backend": "tiled" if lat.algorithm == 2 else "generic"},
             "spin_flips_per_s": flips / (total_ms * 1e-3),
             "back_to_back": {"ns_per_spin_flip": b2b_ms * 1e6 / flips, "ms_per_step": b2b_ms / args.steps, "note": "same K sweeps in one enqueue, warm L2"},
+            "with_measurement": {"ns_per_spin_flip": meas_ms * 1e6 / (args.steps * N), "ms_per_step": meas_ms / args.steps,
+                                 "note": "rank 0: same K sweeps with the integer energy / magnetisation histograms of every configuration (sw_sweep_record)"},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N, "d2h_bytes_per_step": N + 2 * 16 * 8, "steps": e2e_steps},
             "gpu_launches": int(launches),

@@ -83,6 +83,16 @@ int sw_sweep_record(sw_ctx *ctx, int n, int64_t *bond_hist_out, int64_t *state_h
  * Potts energy E/J = 2*L*L - bond_hist[0]; M^2 from state_hist by eq.(3). */
 int sw_observables(sw_ctx *ctx, int64_t *bond_hist, int64_t *state_hist);
 
+/* NEXT-1 of the scope table: the correlation function of PAPER.md eq.(5) at distance r, as an integer histogram
+ * (R15): corr_hist[d] (HOST, q int64) = #{pairs (i, i + r e_x) and (i, i + r e_y), periodic, with
+ * (S_i - S_{i+r}) mod q == d}, 2*L*L pairs, of the current configuration; 0 <= r < L.  The caller derives
+ * G(r) = (1 / 2N) sum_d corr_hist[d] cos(2 pi d / q) (d ascending) and R = G(L/2) / G(L/4) of eq.(6).
+ * sw_sweep_record_corr = sw_sweep_record plus the histograms at the distances r1 and r2 of every configuration
+ * ("+ measurement" of the clock model): four HOST outputs of n*q int64. */
+int sw_correlation(sw_ctx *ctx, int r, int64_t *corr_hist);
+int sw_sweep_record_corr(sw_ctx *ctx, int n, int r1, int r2, int64_t *bond_hist_out, int64_t *state_hist_out,
+                         int64_t *corr1_out, int64_t *corr2_out);
+
 /* Copy the configuration to / from HOST memory (L*L bytes, row-major, values 0..q-1).
  * sw_set_spins also sets the absolute sweep index (resume / oracle hand-off); values >= q are
  * rejected with SW_ERR_ARG and leave the context unchanged. */

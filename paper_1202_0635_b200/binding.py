@@ -37,6 +37,8 @@ SYMBOLS = {
     "sw_sync": (_i, [_vp]),
     "sw_sweep_record": (_i, [_vp, _i, _vp, _vp]),
     "sw_observables": (_i, [_vp, _vp, _vp]),
+    "sw_correlation": (_i, [_vp, _i, _vp]),
+    "sw_sweep_record_corr": (_i, [_vp, _i, _i, _i, _vp, _vp, _vp, _vp]),
     "sw_get_spins": (_i, [_vp, _vp]),
     "sw_set_spins": (_i, [_vp, _vp, _u64]),
     "sw_sweep_index": (_u64, [_vp]),
@@ -160,6 +162,16 @@ class Lattice:
         _check(self._lib.sw_sweep_record(self._h, n, bh.ctypes.data, sh.ctypes.data))
         return bh, sh
 
+    def sweep_record_corr(self, n: int, r1: int, r2: int):
+        out = [np.zeros((n, self.q), dtype=np.int64) for _ in range(4)]
+        _check(self._lib.sw_sweep_record_corr(self._h, n, int(r1), int(r2), *[a.ctypes.data for a in out]))
+        return tuple(out)
+
+    def correlation(self, r: int):
+        ch = np.zeros(self.q, dtype=np.int64)
+        _check(self._lib.sw_correlation(self._h, int(r), ch.ctypes.data))
+        return ch
+
     def observables(self):
         bh = np.zeros(self.q, dtype=np.int64)
         sh = np.zeros(self.q, dtype=np.int64)
@@ -259,6 +271,28 @@ def clock_magnetisation(q: int, state_hist) -> float:
     return math.hypot(mx, my)
 
 
+def correlation_g(q: int, corr_hist) -> float:
+    """G(r) of PAPER.md eq.(5) from the integer histogram: (1 / 2N) sum_d corr_hist[d] cos(2 pi d / q), d ascending."""
+    import math
+    g = 0.0
+    n = 0
+    for d in range(q):
+        g += float(int(corr_hist[d])) * math.cos(2.0 * math.pi * d / q)
+        n += int(corr_hist[d])
+    return g / float(n)
+
+
+def moment_ratio(m2_series) -> float:
+    """U of PAPER.md eq.(2): <M^4> / <M^2>^2 over a series of M^2 values (eq.(3)), accumulated left to right."""
+    s2 = 0.0
+    s4 = 0.0
+    for m2 in m2_series:
+        s2 += float(m2)
+        s4 += float(m2) * float(m2)
+    k = float(len(m2_series))
+    return (s4 / k) / ((s2 / k) * (s2 / k))
+
+
 # The C names, as plain functions over a Lattice (same names as include/sw.h).
 def sw_create(L, q, model, T, seed) -> Lattice:
     return Lattice(L, q, model, T, seed)
@@ -294,3 +328,11 @@ def sw_get_thresholds(ctx: Lattice):
 
 def sw_get_labels(ctx: Lattice):
     return ctx.get_labels()
+
+
+def sw_correlation(ctx: Lattice, r: int):
+    return ctx.correlation(r)
+
+
+def sw_sweep_record_corr(ctx: Lattice, n: int, r1: int, r2: int):
+    return ctx.sweep_record_corr(n, r1, r2)

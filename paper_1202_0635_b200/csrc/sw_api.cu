@@ -40,7 +40,7 @@ int fail(int code, const char *fmt, ...)
 
 constexpr size_t ALIGN = 1024;
 constexpr int REC_ROWS = 512;  // rows of the device ring used by sw_sweep_record
-constexpr int OBS_WORDS = 32;  // [0,16) bond_hist, [16,32) state_hist
+constexpr int OBS_WORDS = 64;  // [0,16) bond_hist, [16,32) state_hist, [32,48) corr_hist(r1), [48,64) corr_hist(r2)
 
 size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
@@ -181,6 +181,15 @@ int launch_observables(sw_ctx *c, unsigned long long *dst)
     return SW_OK;
 }
 
+int launch_correlation(sw_ctx *c, int r, unsigned long long *dst)   // dst: 16 zeroed words
+{
+    const size_t work = (c->L % 4 == 0) ? c->N / 4 : c->N;
+    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 8));
+    sw::k_correlation<<<grid, 256, 0, c->stream>>>(c->md, c->spins, (uint32_t)r, dst);
+    c->launches += 1;
+    return SW_OK;
+}
+
 sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, size_t bytes, void *stream, bool own)
 {
     if (!args_ok(L, q, model) || !(T > 0.0) || !std::isfinite(T)) {
@@ -317,17 +326,23 @@ int sw_sweep(sw_ctx *c, int n)
     return sw_sync(c);
 }
 
-int sw_sweep_record(sw_ctx *c, int n, int64_t *bond_out, int64_t *state_out)
+namespace {
+// n sweeps, row k of every output = the configuration BEFORE the k-th sweep of the call (R10).
+// r1 < 0: no correlation histograms.
+int record_impl(sw_ctx *c, int n, int r1, int r2, int64_t *bond_out, int64_t *state_out, int64_t *c1_out, int64_t *c2_out)
 {
-    if (!c || n < 0 || !bond_out || !state_out) return fail(SW_ERR_ARG, "sw_sweep_record: bad arguments");
-    if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_record: sweep index would exceed 2^32-1");
     std::vector<unsigned long long> host((size_t)REC_ROWS * OBS_WORDS);
     int done = 0;
     while (done < n) {
         const int chunk = std::min(REC_ROWS, n - done);
         for (int k = 0; k < chunk; ++k) {
-            int rc = launch_observables(c, c->ring + (size_t)k * OBS_WORDS);
+            unsigned long long *row = c->ring + (size_t)k * OBS_WORDS;
+            int rc = launch_observables(c, row);
             if (rc != SW_OK) return rc;
+            if (r1 >= 0) {
+                launch_correlation(c, r1, row + 32);
+                launch_correlation(c, r2, row + 48);
+            }
             rc = one_sweep(c);
             if (rc != SW_OK) return rc;
         }
@@ -336,11 +351,46 @@ int sw_sweep_record(sw_ctx *c, int n, int64_t *bond_out, int64_t *state_out)
         CU_TRY(cudaStreamSynchronize(c->stream));
         for (int k = 0; k < chunk; ++k)
             for (int j = 0; j < c->q; ++j) {
-                bond_out[(size_t)(done + k) * c->q + j] = (int64_t)host[(size_t)k * OBS_WORDS + j];
-                state_out[(size_t)(done + k) * c->q + j] = (int64_t)host[(size_t)k * OBS_WORDS + 16 + j];
+                const size_t o = (size_t)(done + k) * c->q + j;
+                bond_out[o] = (int64_t)host[(size_t)k * OBS_WORDS + j];
+                state_out[o] = (int64_t)host[(size_t)k * OBS_WORDS + 16 + j];
+                if (r1 >= 0) {
+                    c1_out[o] = (int64_t)host[(size_t)k * OBS_WORDS + 32 + j];
+                    c2_out[o] = (int64_t)host[(size_t)k * OBS_WORDS + 48 + j];
+                }
             }
         done += chunk;
     }
+    return SW_OK;
+}
+}  // namespace
+
+int sw_sweep_record(sw_ctx *c, int n, int64_t *bond_out, int64_t *state_out)
+{
+    if (!c || n < 0 || !bond_out || !state_out) return fail(SW_ERR_ARG, "sw_sweep_record: bad arguments");
+    if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_record: sweep index would exceed 2^32-1");
+    return record_impl(c, n, -1, -1, bond_out, state_out, nullptr, nullptr);
+}
+
+int sw_sweep_record_corr(sw_ctx *c, int n, int r1, int r2, int64_t *bond_out, int64_t *state_out, int64_t *corr1_out,
+                         int64_t *corr2_out)
+{
+    if (!c || n < 0 || !bond_out || !state_out || !corr1_out || !corr2_out || r1 < 0 || r2 < 0 || r1 >= c->L || r2 >= c->L)
+        return fail(SW_ERR_ARG, "sw_sweep_record_corr: bad arguments (need 0 <= r1, r2 < L and non-NULL outputs)");
+    if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_record_corr: sweep index would exceed 2^32-1");
+    return record_impl(c, n, r1, r2, bond_out, state_out, corr1_out, corr2_out);
+}
+
+int sw_correlation(sw_ctx *c, int r, int64_t *corr_hist)
+{
+    if (!c || !corr_hist || r < 0 || r >= c->L) return fail(SW_ERR_ARG, "sw_correlation: need 0 <= r < L and a non-NULL output");
+    CU_TRY(cudaMemsetAsync(c->obs, 0, 8 * OBS_WORDS, c->stream));
+    launch_correlation(c, r, c->obs + 32);
+    CU_TRY(cudaGetLastError());
+    unsigned long long host[16];
+    CU_TRY(cudaMemcpyAsync(host, c->obs + 32, sizeof(host), cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    for (int j = 0; j < c->q; ++j) corr_hist[j] = (int64_t)host[j];
     return SW_OK;
 }
 

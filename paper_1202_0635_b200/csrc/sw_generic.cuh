@@ -192,6 +192,62 @@ __global__ void __launch_bounds__(256) k_observables(Model md, const uint8_t *__
     }
 }
 
+// Correlation histogram at distance r (eq.(5), (6); R15): out[d] += number of pairs (i, i + r e_x)
+// and (i, i + r e_y), periodic, with (S_i - S_{i+r}) mod q == d (unsigned long long, zeroed by the host).
+// Four sites per thread along x (one 32-bit load each for the site word, the word at x + r when r % 4 == 0, and the
+// word r rows below); per-warp private shared-memory bins, then one global atomic per bin and block.
+__global__ void __launch_bounds__(256) k_correlation(Model md, const uint8_t *__restrict__ spins, uint32_t r,
+                                                     unsigned long long *__restrict__ out)
+{
+    __shared__ unsigned int h[8][16];
+    const int warp = threadIdx.x >> 5;
+    for (int k = threadIdx.x; k < 8 * 16; k += blockDim.x) (&h[0][0])[k] = 0u;
+    __syncthreads();
+    const uint32_t q = (uint32_t)md.q, L = (uint32_t)md.L;
+    if (L % 4u == 0u) {
+        const uint32_t nq = md.N / 4u;
+        for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < nq; g += gridDim.x * blockDim.x) {
+            const uint32_t i = 4u * g, y = i / L, x = i - y * L;
+            uint32_t yd = y + r; if (yd >= L) yd -= L;
+            const uint32_t w = *reinterpret_cast<const uint32_t *>(spins + i);
+            const uint32_t wd = *reinterpret_cast<const uint32_t *>(spins + (size_t)yd * L + x);
+            uint32_t wr;
+            if (r % 4u == 0u) {
+                uint32_t xr = x + r; if (xr >= L) xr -= L;
+                wr = *reinterpret_cast<const uint32_t *>(spins + (size_t)y * L + xr);
+            } else {
+                wr = 0u;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    uint32_t xr = x + (uint32_t)k + r; if (xr >= L) xr -= L;
+                    wr |= (uint32_t)spins[(size_t)y * L + xr] << (8 * k);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t s = (w >> (8 * k)) & 0xFFu, sr = (wr >> (8 * k)) & 0xFFu, sd = (wd >> (8 * k)) & 0xFFu;
+                atomicAdd(&h[warp][s >= sr ? s - sr : s + q - sr], 1u);
+                atomicAdd(&h[warp][s >= sd ? s - sd : s + q - sd], 1u);
+            }
+        }
+    } else {
+        for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < md.N; i += gridDim.x * blockDim.x) {
+            const uint32_t y = i / L, x = i - y * L;
+            uint32_t xr = x + r; if (xr >= L) xr -= L;
+            uint32_t yd = y + r; if (yd >= L) yd -= L;
+            const uint32_t s = spins[i], sr = spins[y * L + xr], sd = spins[yd * L + x];
+            atomicAdd(&h[warp][s >= sr ? s - sr : s + q - sr], 1u);
+            atomicAdd(&h[warp][s >= sd ? s - sd : s + q - sd], 1u);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < 16) {
+        unsigned long long s = 0;
+        for (int w2 = 0; w2 < 8; ++w2) s += h[w2][threadIdx.x];
+        if (s) atomicAdd(out + threadIdx.x, s);
+    }
+}
+
 // Validation of a configuration handed in by sw_set_spins: flag[0] = 1 if any value >= q.
 __global__ void k_check_spins(uint32_t N, uint32_t q, const uint8_t *__restrict__ spins, int *flag)
 {

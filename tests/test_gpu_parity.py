@@ -265,3 +265,47 @@ def test_config5_L16384_three_temperatures(sw, oracle):
     _snapshot_check(sw, oracle, CONFIGS["c5_potts2_L16384_0.8Tc"], early=1, late_at=60, late=1)
     _snapshot_check(sw, oracle, CONFIGS["c5_potts2_L16384_Tc"], early=0, late_at=60, late=1)
     _snapshot_check(sw, oracle, CONFIGS["c5_potts2_L16384_1.2Tc"], early=0, late_at=60, late=1)
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-1: correlation histograms (eq.(5), (6); R15)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,q,model,T", [(64, 6, CLOCK, 0.9), (130, 3, POTTS, tc(3)), (31, 5, CLOCK, 0.7), (256, 2, POTTS, tc(2))])
+def test_correlation_matches_oracle(sw, oracle, L, q, model, T):
+    seed = 0x5EED0C0D
+    with sw.Lattice(L, q, model, T, seed) as lat:
+        lat.sweep(3)
+        s = lat.get_spins()
+        for r in sorted({0, 1, 2, 3, L // 4, L // 2, L - 1}):
+            _assert_same(lat.correlation(r), oracle.correlation(L, q, s, r), f"corr_hist r={r}")
+        bh, _ = lat.observables()
+        _assert_same(lat.correlation(1), bh, "corr_hist(1) == bond_hist")
+        with pytest.raises(sw.SwError):
+            lat.correlation(L)
+
+
+def test_record_corr_rows_and_derived_doubles(sw, oracle):
+    L, q, T, seed, n = 128, 6, 0.9, 0x5EED0C0E, 6
+    with sw.Lattice(L, q, CLOCK, T, seed) as lat:
+        bh, sh, c1, c2 = lat.sweep_record_corr(n, L // 4, L // 2)
+    s = oracle.init_spins(L, q, seed)
+    for k in range(n):
+        obh, osh = oracle.observables(L, q, s)
+        _assert_same(bh[k], obh, f"bond row {k}")
+        _assert_same(sh[k], osh, f"state row {k}")
+        o1, o2 = oracle.correlation(L, q, s, L // 4), oracle.correlation(L, q, s, L // 2)
+        _assert_same(c1[k], o1, f"corr(L/4) row {k}")
+        _assert_same(c2[k], o2, f"corr(L/2) row {k}")
+        g1, g2 = sw.correlation_g(q, c1[k]), sw.correlation_g(q, o1)
+        assert g1 == g2 and abs(g1) <= 1.0
+        s = oracle.sweep(L, q, CLOCK, T, seed, k, s)
+
+
+def test_correlation_full_size_sampled(sw, oracle):
+    """L=4096 clock lattice (config 3 shape): the full histogram at r = L/4 and L/2 against the oracle."""
+    L, q, T, seed = 4096, 6, 0.9, 0x5EED0003
+    with sw.Lattice(L, q, CLOCK, T, seed) as lat:
+        lat.sweep(20)
+        s = lat.get_spins()
+        for r in (L // 4, L // 2, 5):
+            _assert_same(lat.correlation(r), oracle.correlation(L, q, s, r), f"corr_hist r={r}")
