@@ -172,11 +172,12 @@ int one_sweep(sw_ctx *c, cudaEvent_t *ev = nullptr)
     return rc;
 }
 
-int launch_observables(sw_ctx *c, unsigned long long *dst)
+int launch_observables(sw_ctx *c, unsigned long long *dst, bool zero = true)   // dst: one row of OBS_WORDS words
 {
-    CU_TRY(cudaMemsetAsync(dst, 0, 8 * OBS_WORDS, c->stream));
-    const unsigned grid = (unsigned)std::min<size_t>((c->N + 255) / 256, 148 * 8);
-    sw::k_observables<<<grid, 256, 0, c->stream>>>(c->md, c->spins, dst);
+    if (zero) CU_TRY(cudaMemsetAsync(dst, 0, 8 * OBS_WORDS, c->stream));
+    const size_t work = (c->L % 16 == 0) ? c->N / 16 : c->N;
+    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 6));
+    sw::launch_pdl(sw::k_observables, grid, sw::HIST_THREADS, c->stream, c->md, (const uint8_t *)c->spins, dst);
     c->launches += 1;
     return SW_OK;
 }
@@ -184,8 +185,8 @@ int launch_observables(sw_ctx *c, unsigned long long *dst)
 int launch_correlation(sw_ctx *c, int r, unsigned long long *dst)   // dst: 16 zeroed words
 {
     const size_t work = (c->L % 4 == 0) ? c->N / 4 : c->N;
-    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 8));
-    sw::k_correlation<<<grid, 256, 0, c->stream>>>(c->md, c->spins, (uint32_t)r, dst);
+    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 6));
+    sw::launch_pdl(sw::k_correlation, grid, sw::HIST_THREADS, c->stream, c->md, (const uint8_t *)c->spins, (uint32_t)r, dst);
     c->launches += 1;
     return SW_OK;
 }
@@ -335,9 +336,10 @@ int record_impl(sw_ctx *c, int n, int r1, int r2, int64_t *bond_out, int64_t *st
     int done = 0;
     while (done < n) {
         const int chunk = std::min(REC_ROWS, n - done);
+        CU_TRY(cudaMemsetAsync(c->ring, 0, (size_t)chunk * OBS_WORDS * 8, c->stream));   // all rows of the chunk at once
         for (int k = 0; k < chunk; ++k) {
             unsigned long long *row = c->ring + (size_t)k * OBS_WORDS;
-            int rc = launch_observables(c, row);
+            int rc = launch_observables(c, row, false);
             if (rc != SW_OK) return rc;
             if (r1 >= 0) {
                 launch_correlation(c, r1, row + 32);

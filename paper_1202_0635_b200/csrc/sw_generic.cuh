@@ -9,10 +9,35 @@
 // It is the slow, simple path: the tiled back-end replaces S1/S2/S3 for L % 128 == 0 and is checked
 // against this one on the device as well as against the oracle.
 #pragma once
+#include <cuda_runtime.h>
 #include <stdint.h>
 #include "sw_philox.cuh"
 
 namespace sw {
+
+// Programmatic dependent launch: every kernel of the sweep lets the next one be scheduled early (its CTAs become
+// resident while this grid drains) and itself waits here until the previous grid has completed and flushed.
+__device__ __forceinline__ void pdl_prologue()
+{
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
+template <typename... Params, typename... Args>
+static inline void launch_pdl(void (*kernel)(Params...), unsigned grid, unsigned block, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
+}
 
 struct Model {
     int L;
@@ -162,51 +187,111 @@ __global__ void k_flip(Model md, PhiloxKey key, uint32_t t, const int32_t *__res
     }
 }
 
-// S5.  out[0..q) += bond_hist, out[16..16+q) += state_hist (unsigned long long, zeroed by the host).
-// Per-warp private shared-memory histograms, then one global atomic per bin per block.
-__global__ void __launch_bounds__(256) k_observables(Model md, const uint8_t *__restrict__ spins,
-                                                     unsigned long long *__restrict__ out)
+// S5 and the correlation histograms.  Both kernels count into per-thread private columns of a shared-memory table
+// ([bin][thread]: conflict-free plain increments, no atomics -- with q = 2 a warp-wide shared atomic would serialise
+// 16-fold on two addresses), four sites per thread and iteration with 32-bit loads, then one reduction per block and
+// one global atomic per bin and block.  L % 4 != 0 (small odd lattices, generic back-end only) takes a plain path.
+constexpr int HIST_THREADS = 256;
+
+__device__ __forceinline__ uint32_t diff_mod_q(uint32_t s, uint32_t o, uint32_t q) { return s >= o ? s - o : s + q - o; }
+
+// sum the NB bins over the block's threads and add them to out[0..NB)
+template <int NB>
+__device__ __forceinline__ void hist_flush(unsigned int (*h)[HIST_THREADS], unsigned long long *__restrict__ out)
 {
-    __shared__ unsigned int h[8][32];
-    const int warp = threadIdx.x >> 5;
-    for (int k = threadIdx.x; k < 8 * 32; k += blockDim.x) (&h[0][0])[k] = 0u;
     __syncthreads();
-    const uint32_t q = (uint32_t)md.q;
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < md.N; i += gridDim.x * blockDim.x) {
-        const uint32_t y = i / (uint32_t)md.L, x = i - y * (uint32_t)md.L;
-        const uint32_t xr = (x + 1u == (uint32_t)md.L) ? 0u : x + 1u;
-        const uint32_t yd = (y + 1u == (uint32_t)md.L) ? 0u : y + 1u;
-        const uint32_t s = spins[i];
-        const uint32_t sr = spins[y * md.L + xr], sd = spins[yd * md.L + x];
-        const uint32_t d0 = s >= sr ? s - sr : s + q - sr;
-        const uint32_t d1 = s >= sd ? s - sd : s + q - sd;
-        atomicAdd(&h[warp][d0], 1u);
-        atomicAdd(&h[warp][d1], 1u);
-        atomicAdd(&h[warp][16u + s], 1u);
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    for (uint32_t b = warp; b < (uint32_t)NB; b += HIST_THREADS / 32) {
+        uint32_t v = 0u;
+        for (uint32_t k = lane; k < (uint32_t)HIST_THREADS; k += 32u) v += h[b][k];
+        v = __reduce_add_sync(0xFFFFFFFFu, v);
+        if (lane == 0u && v) atomicAdd(out + b, (unsigned long long)v);
     }
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        unsigned long long s = 0;
-        for (int w2 = 0; w2 < 8; ++w2) s += h[w2][threadIdx.x];
-        if (s) atomicAdd(out + threadIdx.x, s);
+}
+
+// byte-wise (a - b) mod q of two words of four spins (all bytes < q <= 16)
+__device__ __forceinline__ uint32_t diff4_mod_q(uint32_t a, uint32_t b, uint32_t q)
+{
+    uint32_t t = a + q * 0x01010101u - b;                                   // bytes in [1, 2q - 1]: no borrow between bytes
+    const uint32_t ge = (t + (0x80u - q) * 0x01010101u) & 0x80808080u;      // bit 7 of a byte set <=> byte >= q
+    return t - (ge >> 7) * q;
+}
+// number of bytes of v (all < 32) that differ from d
+__device__ __forceinline__ uint32_t bytes_ne(uint32_t v, uint32_t d)
+{
+    return (uint32_t)__popc(((v ^ (d * 0x01010101u)) + 0x7F7F7F7Fu) & 0x80808080u);
+}
+
+// out[0..q) += bond_hist, out[16..16+q) += state_hist (unsigned long long, zeroed by the host).
+// L % 4 == 0: four sites per thread and iteration, counted in registers with byte-parallel compares (one counter
+// per value d < q; the loop over d is unrolled and cut off by the uniform test d < q), no shared-memory traffic.
+__global__ void __launch_bounds__(HIST_THREADS) k_observables(Model md, const uint8_t *__restrict__ spins,
+                                                              unsigned long long *__restrict__ out)
+{
+    __shared__ unsigned int h[32][HIST_THREADS];
+    const uint32_t tid = threadIdx.x;
+    pdl_prologue();
+    const uint32_t q = (uint32_t)md.q, L = (uint32_t)md.L;
+    if (L % 16u == 0u) {
+        uint32_t nb[16], ns[16], groups = 0u;        // bytes NOT equal to d, summed; turned into counts at the end
+#pragma unroll
+        for (int d = 0; d < 16; ++d) nb[d] = ns[d] = 0u;
+        const uint32_t nq = md.N / 16u;              // 16 sites (one 128-bit load) per thread and iteration
+        for (uint32_t g = blockIdx.x * blockDim.x + tid; g < nq; g += gridDim.x * blockDim.x) {
+            const uint32_t i = 16u * g, y = i / L, x = i - y * L;
+            const uint32_t yd = (y + 1u == L) ? 0u : y + 1u, xr = (x + 16u == L) ? 0u : x + 16u;
+            const uint4 w4 = *reinterpret_cast<const uint4 *>(spins + i);
+            const uint4 d4 = *reinterpret_cast<const uint4 *>(spins + (size_t)yd * L + x);
+            const uint32_t nx = spins[(size_t)y * L + xr];
+            const uint32_t w[4] = { w4.x, w4.y, w4.z, w4.w }, wd[4] = { d4.x, d4.y, d4.z, d4.w };
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const uint32_t wr = (w[c] >> 8) | ((c < 3 ? w[c < 3 ? c + 1 : 3] : nx) << 24);
+                const uint32_t dh = diff4_mod_q(w[c], wr, q), dv = diff4_mod_q(w[c], wd[c], q);
+#pragma unroll
+                for (int d = 0; d < 16; ++d) {
+                    if ((uint32_t)d < q) {
+                        nb[d] += bytes_ne(dh, (uint32_t)d) + bytes_ne(dv, (uint32_t)d);
+                        ns[d] += bytes_ne(w[c], (uint32_t)d);
+                    }
+                }
+            }
+            groups += 4u;
+        }
+#pragma unroll
+        for (int d = 0; d < 16; ++d) {
+            h[d][tid] = ((uint32_t)d < q) ? 8u * groups - nb[d] : 0u;
+            h[16 + d][tid] = ((uint32_t)d < q) ? 4u * groups - ns[d] : 0u;
+        }
+    } else {
+        for (int b = 0; b < 32; ++b) h[b][tid] = 0u;
+        for (uint32_t i = blockIdx.x * blockDim.x + tid; i < md.N; i += gridDim.x * blockDim.x) {
+            const uint32_t y = i / L, x = i - y * L;
+            const uint32_t xr = (x + 1u == L) ? 0u : x + 1u, yd = (y + 1u == L) ? 0u : y + 1u;
+            const uint32_t s = spins[i];
+            h[diff_mod_q(s, spins[y * L + xr], q)][tid] += 1u;
+            h[diff_mod_q(s, spins[yd * L + x], q)][tid] += 1u;
+            h[16u + s][tid] += 1u;
+        }
     }
+    hist_flush<32>(h, out);
 }
 
 // Correlation histogram at distance r (eq.(5), (6); R15): out[d] += number of pairs (i, i + r e_x)
 // and (i, i + r e_y), periodic, with (S_i - S_{i+r}) mod q == d (unsigned long long, zeroed by the host).
-// Four sites per thread along x (one 32-bit load each for the site word, the word at x + r when r % 4 == 0, and the
-// word r rows below); per-warp private shared-memory bins, then one global atomic per bin and block.
-__global__ void __launch_bounds__(256) k_correlation(Model md, const uint8_t *__restrict__ spins, uint32_t r,
-                                                     unsigned long long *__restrict__ out)
+__global__ void __launch_bounds__(HIST_THREADS) k_correlation(Model md, const uint8_t *__restrict__ spins, uint32_t r,
+                                                              unsigned long long *__restrict__ out)
 {
-    __shared__ unsigned int h[8][16];
-    const int warp = threadIdx.x >> 5;
-    for (int k = threadIdx.x; k < 8 * 16; k += blockDim.x) (&h[0][0])[k] = 0u;
-    __syncthreads();
+    __shared__ unsigned int h[16][HIST_THREADS];
+    const uint32_t tid = threadIdx.x;
+    pdl_prologue();
     const uint32_t q = (uint32_t)md.q, L = (uint32_t)md.L;
     if (L % 4u == 0u) {
+        uint32_t nb[16], groups = 0u;
+#pragma unroll
+        for (int d = 0; d < 16; ++d) nb[d] = 0u;
         const uint32_t nq = md.N / 4u;
-        for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < nq; g += gridDim.x * blockDim.x) {
+        for (uint32_t g = blockIdx.x * blockDim.x + tid; g < nq; g += gridDim.x * blockDim.x) {
             const uint32_t i = 4u * g, y = i / L, x = i - y * L;
             uint32_t yd = y + r; if (yd >= L) yd -= L;
             const uint32_t w = *reinterpret_cast<const uint32_t *>(spins + i);
@@ -223,29 +308,26 @@ __global__ void __launch_bounds__(256) k_correlation(Model md, const uint8_t *__
                     wr |= (uint32_t)spins[(size_t)y * L + xr] << (8 * k);
                 }
             }
+            const uint32_t dh = diff4_mod_q(w, wr, q), dv = diff4_mod_q(w, wd, q);
+            ++groups;
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const uint32_t s = (w >> (8 * k)) & 0xFFu, sr = (wr >> (8 * k)) & 0xFFu, sd = (wd >> (8 * k)) & 0xFFu;
-                atomicAdd(&h[warp][s >= sr ? s - sr : s + q - sr], 1u);
-                atomicAdd(&h[warp][s >= sd ? s - sd : s + q - sd], 1u);
-            }
+            for (int d = 0; d < 16; ++d)
+                if ((uint32_t)d < q) nb[d] += bytes_ne(dh, (uint32_t)d) + bytes_ne(dv, (uint32_t)d);
         }
+#pragma unroll
+        for (int d = 0; d < 16; ++d) h[d][tid] = ((uint32_t)d < q) ? 8u * groups - nb[d] : 0u;
     } else {
-        for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < md.N; i += gridDim.x * blockDim.x) {
+        for (int b = 0; b < 16; ++b) h[b][tid] = 0u;
+        for (uint32_t i = blockIdx.x * blockDim.x + tid; i < md.N; i += gridDim.x * blockDim.x) {
             const uint32_t y = i / L, x = i - y * L;
             uint32_t xr = x + r; if (xr >= L) xr -= L;
             uint32_t yd = y + r; if (yd >= L) yd -= L;
-            const uint32_t s = spins[i], sr = spins[y * L + xr], sd = spins[yd * L + x];
-            atomicAdd(&h[warp][s >= sr ? s - sr : s + q - sr], 1u);
-            atomicAdd(&h[warp][s >= sd ? s - sd : s + q - sd], 1u);
+            const uint32_t s = spins[i];
+            h[diff_mod_q(s, spins[y * L + xr], q)][tid] += 1u;
+            h[diff_mod_q(s, spins[yd * L + x], q)][tid] += 1u;
         }
     }
-    __syncthreads();
-    if (threadIdx.x < 16) {
-        unsigned long long s = 0;
-        for (int w2 = 0; w2 < 8; ++w2) s += h[w2][threadIdx.x];
-        if (s) atomicAdd(out + threadIdx.x, s);
-    }
+    hist_flush<16>(h, out);
 }
 
 // Validation of a configuration handed in by sw_set_spins: flag[0] = 1 if any value >= q.

@@ -77,30 +77,6 @@ static inline size_t tiled_workspace_bytes(int L)
            tiles * ECNT * 2 + 1024 + tiles * 4 + 1024;
 }
 
-// Programmatic dependent launch: every kernel of the sweep lets the next one be scheduled early (its CTAs become
-// resident while this grid drains) and itself waits here until the previous grid has completed and flushed.
-__device__ __forceinline__ void pdl_prologue()
-{
-    asm volatile("griddepcontrol.launch_dependents;");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-}
-
-template <typename... Params, typename... Args>
-static inline void launch_pdl(void (*kernel)(Params...), unsigned grid, unsigned block, cudaStream_t stream, Args... args)
-{
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(block);
-    cfg.dynamicSmemBytes = 0;
-    cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
-}
-
 // ---- shared-memory union-find by minimum index (same scheme as uf_union in sw_generic.cuh) ------------------
 __device__ __forceinline__ uint32_t sfind_halve(volatile uint32_t *lab, uint32_t a)
 {
