@@ -176,7 +176,7 @@ int launch_observables(sw_ctx *c, unsigned long long *dst, bool zero = true)   /
 {
     if (zero) CU_TRY(cudaMemsetAsync(dst, 0, 8 * OBS_WORDS, c->stream));
     const size_t work = (c->L % 16 == 0) ? c->N / 16 : c->N;
-    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 6));
+    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 4));
     sw::launch_pdl(sw::k_observables, grid, sw::HIST_THREADS, c->stream, c->md, (const uint8_t *)c->spins, dst);
     c->launches += 1;
     return SW_OK;
