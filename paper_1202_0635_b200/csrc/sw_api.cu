@@ -177,16 +177,25 @@ int launch_observables(sw_ctx *c, unsigned long long *dst, bool zero = true)   /
     if (zero) CU_TRY(cudaMemsetAsync(dst, 0, 8 * OBS_WORDS, c->stream));
     const size_t work = (c->L % 16 == 0) ? c->N / 16 : c->N;
     const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 4));
-    sw::launch_pdl(sw::k_observables, grid, sw::HIST_THREADS, c->stream, c->md, (const uint8_t *)c->spins, dst);
+    const uint8_t *sp = c->spins;
+    if (c->q <= 2) sw::launch_pdl(sw::k_observables<2>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
+    else if (c->q <= 4) sw::launch_pdl(sw::k_observables<4>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
+    else if (c->q <= 8) sw::launch_pdl(sw::k_observables<8>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
+    else sw::launch_pdl(sw::k_observables<16>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
     c->launches += 1;
     return SW_OK;
 }
 
 int launch_correlation(sw_ctx *c, int r, unsigned long long *dst)   // dst: 16 zeroed words
 {
-    const size_t work = (c->L % 4 == 0) ? c->N / 4 : c->N;
-    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 6));
-    sw::launch_pdl(sw::k_correlation, grid, sw::HIST_THREADS, c->stream, c->md, (const uint8_t *)c->spins, (uint32_t)r, dst);
+    const size_t work = (c->L % 16 == 0 && r % 4 == 0) ? c->N / 16 : (c->L % 4 == 0) ? c->N / 4 : c->N;
+    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 4));
+    const uint8_t *sp = c->spins;
+    const uint32_t ur = (uint32_t)r;
+    if (c->q <= 2) sw::launch_pdl(sw::k_correlation<2>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
+    else if (c->q <= 4) sw::launch_pdl(sw::k_correlation<4>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
+    else if (c->q <= 8) sw::launch_pdl(sw::k_correlation<8>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
+    else sw::launch_pdl(sw::k_correlation<16>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
     c->launches += 1;
     return SW_OK;
 }

@@ -225,6 +225,7 @@ __device__ __forceinline__ uint32_t bytes_ne(uint32_t v, uint32_t d)
 // out[0..q) += bond_hist, out[16..16+q) += state_hist (unsigned long long, zeroed by the host).
 // L % 4 == 0: four sites per thread and iteration, counted in registers with byte-parallel compares (one counter
 // per value d < q; the loop over d is unrolled and cut off by the uniform test d < q), no shared-memory traffic.
+template <int QB>   // QB = 2, 4, 8 or 16 >= q: bound of the unrolled loops over the values d
 __global__ void __launch_bounds__(HIST_THREADS) k_observables(Model md, const uint8_t *__restrict__ spins,
                                                               unsigned long long *__restrict__ out)
 {
@@ -235,7 +236,7 @@ __global__ void __launch_bounds__(HIST_THREADS) k_observables(Model md, const ui
     if (L % 16u == 0u) {
         uint32_t nb[16], ns[16], groups = 0u;        // bytes NOT equal to d, summed; turned into counts at the end
 #pragma unroll
-        for (int d = 0; d < 16; ++d) nb[d] = ns[d] = 0u;
+        for (int d = 0; d < QB; ++d) nb[d] = ns[d] = 0u;
         const uint32_t nq = md.N / 16u;              // 16 sites (one 128-bit load) per thread and iteration
         for (uint32_t g = blockIdx.x * blockDim.x + tid; g < nq; g += gridDim.x * blockDim.x) {
             const uint32_t i = 16u * g, y = i / L, x = i - y * L;
@@ -249,7 +250,7 @@ __global__ void __launch_bounds__(HIST_THREADS) k_observables(Model md, const ui
                 const uint32_t wr = (w[c] >> 8) | ((c < 3 ? w[c < 3 ? c + 1 : 3] : nx) << 24);
                 const uint32_t dh = diff4_mod_q(w[c], wr, q), dv = diff4_mod_q(w[c], wd[c], q);
 #pragma unroll
-                for (int d = 0; d < 16; ++d) {
+                for (int d = 0; d < QB; ++d) {
                     if ((uint32_t)d < q) {
                         nb[d] += bytes_ne(dh, (uint32_t)d) + bytes_ne(dv, (uint32_t)d);
                         ns[d] += bytes_ne(w[c], (uint32_t)d);
@@ -258,8 +259,9 @@ __global__ void __launch_bounds__(HIST_THREADS) k_observables(Model md, const ui
             }
             groups += 4u;
         }
+        for (int b2 = 0; b2 < 32; ++b2) h[b2][tid] = 0u;
 #pragma unroll
-        for (int d = 0; d < 16; ++d) {
+        for (int d = 0; d < QB; ++d) {
             h[d][tid] = ((uint32_t)d < q) ? 8u * groups - nb[d] : 0u;
             h[16 + d][tid] = ((uint32_t)d < q) ? 4u * groups - ns[d] : 0u;
         }
@@ -279,6 +281,7 @@ __global__ void __launch_bounds__(HIST_THREADS) k_observables(Model md, const ui
 
 // Correlation histogram at distance r (eq.(5), (6); R15): out[d] += number of pairs (i, i + r e_x)
 // and (i, i + r e_y), periodic, with (S_i - S_{i+r}) mod q == d (unsigned long long, zeroed by the host).
+template <int QB>
 __global__ void __launch_bounds__(HIST_THREADS) k_correlation(Model md, const uint8_t *__restrict__ spins, uint32_t r,
                                                               unsigned long long *__restrict__ out)
 {
@@ -286,10 +289,40 @@ __global__ void __launch_bounds__(HIST_THREADS) k_correlation(Model md, const ui
     const uint32_t tid = threadIdx.x;
     pdl_prologue();
     const uint32_t q = (uint32_t)md.q, L = (uint32_t)md.L;
-    if (L % 4u == 0u) {
+    if (L % 16u == 0u && r % 4u == 0u) {
+        // 16 sites per thread and iteration (the distances the paper measures, L/4 and L/2, take this path)
         uint32_t nb[16], groups = 0u;
 #pragma unroll
-        for (int d = 0; d < 16; ++d) nb[d] = 0u;
+        for (int d = 0; d < QB; ++d) nb[d] = 0u;
+        const uint32_t nq = md.N / 16u;
+        for (uint32_t g = blockIdx.x * blockDim.x + tid; g < nq; g += gridDim.x * blockDim.x) {
+            const uint32_t i = 16u * g, y = i / L, x = i - y * L;
+            uint32_t yd = y + r; if (yd >= L) yd -= L;
+            const uint4 w4 = *reinterpret_cast<const uint4 *>(spins + i);
+            const uint4 d4 = *reinterpret_cast<const uint4 *>(spins + (size_t)yd * L + x);
+            uint32_t wr[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                uint32_t xr = x + 4u * (uint32_t)c + r; if (xr >= L) xr -= L;
+                wr[c] = *reinterpret_cast<const uint32_t *>(spins + (size_t)y * L + xr);
+            }
+            const uint32_t w[4] = { w4.x, w4.y, w4.z, w4.w }, wd[4] = { d4.x, d4.y, d4.z, d4.w };
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const uint32_t dh = diff4_mod_q(w[c], wr[c], q), dv = diff4_mod_q(w[c], wd[c], q);
+#pragma unroll
+                for (int d = 0; d < QB; ++d)
+                    if ((uint32_t)d < q) nb[d] += bytes_ne(dh, (uint32_t)d) + bytes_ne(dv, (uint32_t)d);
+            }
+            groups += 4u;
+        }
+        for (int b2 = 0; b2 < 16; ++b2) h[b2][tid] = 0u;
+#pragma unroll
+        for (int d = 0; d < QB; ++d) h[d][tid] = ((uint32_t)d < q) ? 8u * groups - nb[d] : 0u;
+    } else if (L % 4u == 0u) {
+        uint32_t nb[16], groups = 0u;
+#pragma unroll
+        for (int d = 0; d < QB; ++d) nb[d] = 0u;
         const uint32_t nq = md.N / 4u;
         for (uint32_t g = blockIdx.x * blockDim.x + tid; g < nq; g += gridDim.x * blockDim.x) {
             const uint32_t i = 4u * g, y = i / L, x = i - y * L;
@@ -311,11 +344,12 @@ __global__ void __launch_bounds__(HIST_THREADS) k_correlation(Model md, const ui
             const uint32_t dh = diff4_mod_q(w, wr, q), dv = diff4_mod_q(w, wd, q);
             ++groups;
 #pragma unroll
-            for (int d = 0; d < 16; ++d)
+            for (int d = 0; d < QB; ++d)
                 if ((uint32_t)d < q) nb[d] += bytes_ne(dh, (uint32_t)d) + bytes_ne(dv, (uint32_t)d);
         }
+        for (int b2 = 0; b2 < 16; ++b2) h[b2][tid] = 0u;
 #pragma unroll
-        for (int d = 0; d < 16; ++d) h[d][tid] = ((uint32_t)d < q) ? 8u * groups - nb[d] : 0u;
+        for (int d = 0; d < QB; ++d) h[d][tid] = ((uint32_t)d < q) ? 8u * groups - nb[d] : 0u;
     } else {
         for (int b = 0; b < 16; ++b) h[b][tid] = 0u;
         for (uint32_t i = blockIdx.x * blockDim.x + tid; i < md.N; i += gridDim.x * blockDim.x) {
