@@ -276,7 +276,7 @@ def main():
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        Ls, ns_sw = min(L, 2048), 3
+        Ls, ns_sw = min(L, 4096), 12     # ~15 s of one host core at ~70 ns per spin
         ns, dt = oracle_ns_per_spin(Ls, q, w.model, w.T, w.seed, ns_sw, 1)
         cpu = {"value": ns, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"{ns_sw} oracle sweeps of an L={Ls} lattice of the same model and T after 1 warm-up sweep ({dt:.1f} s)"}
