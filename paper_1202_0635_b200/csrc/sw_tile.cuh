@@ -417,20 +417,36 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     {
         volatile uint32_t *vl = s_lab;
         uint32_t rall = 0u;                       // this word's roots (their entries: sp, or sp | LOPEN when open)
-        for (uint32_t c = cs; c; c &= c - 1u) {
+        uint32_t cand = cs;
+        if (MODEL == 1) {
+            // A spin on the mirror axis has no active bond at all (its thresholds are 0, R4) and the
+            // reflection maps it to itself: a closed singleton whose decision is never used -- no draw.  At most two
+            // states lie on the axis (2 s = m mod q); ax = the word's sites in one of them, by zero-byte tests on the
+            // word's 32 spins (0x1F: no such state).
+            const uint32_t q = (uint32_t)md.q;
+            uint32_t a1 = 0x1Fu, a2 = 0x1Fu;
+            if ((m & 1u) == 0u) { a1 = m >> 1; if ((q & 1u) == 0u) a2 = (m + q) >> 1; }
+            else if (q & 1u) a1 = (m + q) >> 1;
+            const uint4 *sp4 = reinterpret_cast<const uint4 *>(spins + (size_t)(y0 + wy) * L + x0 + ww * 32u);
+            const uint4 lo = sp4[0], hi = sp4[1];
+            const uint32_t wv[8] = { lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w };
+            uint32_t ax = 0u;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const uint32_t z = (~((wv[j] ^ (a1 * 0x01010101u)) + 0x7F7F7F7Fu) | ~((wv[j] ^ (a2 * 0x01010101u)) + 0x7F7F7F7Fu)) &
+                                   0x80808080u;                      // bit 7 of a byte set <=> that spin is on the axis
+                ax |= ((z * 0x00204081u) >> 28) << (4 * j);          // bits 7, 15, 23, 31 -> one nibble
+            }
+            cand &= ~ax;
+            for (; ax; ax &= ax - 1u) {
+                const uint32_t k = (uint32_t)__ffs((int)ax) - 1u;
+                vl[sb + k] = (sb + k) | ((fuse ? (uint32_t)DEC_BASE : sb + k) << 16);
+            }
+        }
+        for (uint32_t c = cand; c; c &= c - 1u) {
             const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
             const uint32_t v = vl[sb + k];
-            if ((v & LMASK) == sb + k) {
-                bool on_axis = false;
-                if (MODEL == 1) {
-                    // a spin on the mirror axis has no active bond at all (its thresholds are 0, R4) and the
-                    // reflection maps it to itself: a closed singleton whose decision is never used -- no draw
-                    const uint32_t c = clock_c(spins[(size_t)(y0 + wy) * L + x0 + ww * 32u + k], m, q2);
-                    on_axis = (c == 0u) || (c == (uint32_t)md.q);
-                }
-                if (on_axis) vl[sb + k] = (sb + k) | ((fuse ? (uint32_t)DEC_BASE : sb + k) << 16);
-                else rall |= 1u << k;
-            }
+            if ((v & LMASK) == sb + k) rall |= 1u << k;
         }
         // compact the warp's roots into its list (reusing the second half of the warp's edge list), so that the
         // decisions are drawn -- and the open roots registered -- with all lanes busy
