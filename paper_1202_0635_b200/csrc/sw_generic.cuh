@@ -55,6 +55,14 @@ __device__ __forceinline__ uint32_t clock_c(uint32_t s, uint32_t m, uint32_t q2)
     return c >= q2 ? c - q2 : c;
 }
 
+// the same for the four spins of a word (bytes < q <= 16): 2 s + 2q - m <= 62 per byte, no carry between bytes
+__device__ __forceinline__ uint32_t clock_c4(uint32_t w, uint32_t m, uint32_t q2)
+{
+    const uint32_t t = 2u * w + (q2 - m) * 0x01010101u;
+    const uint32_t ge = (t + (0x80u - q2) * 0x01010101u) & 0x80808080u;   // bit 7 of a byte set <=> byte >= 2q
+    return t - (ge >> 7) * q2;
+}
+
 __global__ void k_init_spins(Model md, PhiloxKey key, uint8_t *__restrict__ spins)
 {
     const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;  // group of 4 sites

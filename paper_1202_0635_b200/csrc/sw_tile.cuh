@@ -170,6 +170,11 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             if (gy == L) gy = 0u;
             row[j] = *reinterpret_cast<const uint32_t *>(spins + (size_t)gy * L + gx);
             if (j < ROWS_PER_WARP) hal[j] = (lane == 31u) ? (uint32_t)spins[(size_t)gy * L + xr] : 0u;
+            if (MODEL == 1) {
+                // clock: work on c = (2 s - m) mod 2q from here on (R4), four bytes at a time
+                row[j] = clock_c4(row[j], m, q2);
+                if (j < ROWS_PER_WARP) hal[j] = clock_c4(hal[j], m, q2) & 0xFFu;
+            }
         }
 #pragma unroll
         for (int j = 0; j < ROWS_PER_WARP; ++j) {
@@ -196,9 +201,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             } else {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                    const uint32_t c = clock_c((cur >> (8 * k)) & 0xFFu, m, q2);
-                    const uint32_t cr = clock_c((right >> (8 * k)) & 0xFFu, m, q2);
-                    const uint32_t cd = clock_c((nxt >> (8 * k)) & 0xFFu, m, q2);
+                    const uint32_t c = (cur >> (8 * k)) & 0xFFu, cr = (right >> (8 * k)) & 0xFFu, cd = (nxt >> (8 * k)) & 0xFFu;
                     const uint32_t wh = (k < 2) ? wa[2 * k] : wb[2 * (k - 2)];
                     const uint32_t wv = (k < 2) ? wa[2 * k + 1] : wb[2 * (k - 2) + 1];
                     hn |= (wh < s_table[c * q2 + cr]) ? (1u << k) : 0u;
