@@ -1,5 +1,5 @@
 // libsw.so -- C ABI of include/sw.h: context, host-side scheduling of the sweep kernels, copies.
-// All arithmetic of the method runs in the kernels of sw_generic.cuh / sw_tiled.cuh; the only host
+// All arithmetic of the method runs in the kernels of sw_generic.cuh / sw_tile.cuh; the only host
 // arithmetic is the threshold table (double precision, once per context; R6/R7).
 #include <cuda_runtime.h>
 
