@@ -8,10 +8,11 @@
  * --impl reference legs may build, load or call this file.  It shares no code, header, table or
  * helper with the CUDA path under paper_1202_0635_b200/csrc/.
  *
- * Where the paper is silent the readings of DESIGN.md section 3 (R1..R14) are used; each is
+ * Where the paper is silent the readings of DESIGN.md section 3 (R1..R15) are used; each is
  * cited at its point of use.  Parity status: every function below is pinned by tests/ (Philox
  * known answers, high-precision thresholds, brute-force flood fill, exact enumeration of the
- * Boltzmann distribution on small tori, Kaufman/Onsager energy) -- nothing is "parity unpinned".
+ * Boltzmann distribution on small tori, Kaufman/Onsager energy; oracle_correlation: tests/test_oracle_corr_pins.py)
+ * -- nothing is "parity unpinned".
  *
  * Conventions: N = L*L, site i = y*L + x (x fastest).  Each site owns two bonds:
  * direction 0 to (x+1 mod L, y) and direction 1 to (x, y+1 mod L)  (periodic; R8).
