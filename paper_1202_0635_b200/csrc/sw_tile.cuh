@@ -116,6 +116,11 @@ __device__ __forceinline__ uint32_t root_site(uint32_t v, uint32_t X0, uint32_t 
     return (Y0 + p / TW) * L + X0 + p % TW;
 }
 
+// g = 2 g + [w >= th], th > 0, nth = 2^32 - th: the carry of w + nth shifted into g
+__device__ __forceinline__ void ge_shift_in(uint32_t &g, uint32_t w, uint32_t nth)
+{
+    asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(g) : "r"(w), "r"(nth));
+}
 // K1.  grid = tiles, block = TILE_THREADS.  MODEL 0 = Potts, 1 = clock.
 #ifndef SW_LABEL_MINB
 #define SW_LABEL_MINB 5
@@ -164,6 +169,9 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         const uint32_t xr = (x0 + TW == L) ? 0u : x0 + TW;   // halo column (periodic)
         const uint32_t ly0 = warp * ROWS_PER_WARP;
         uint32_t row[ROWS_PER_WARP + 1], hal[ROWS_PER_WARP];
+        const uint32_t nth = 0u - md.thr_potts;                           // 2^32 - threshold (mod 2^32)
+        const uint32_t emask = md.thr_potts ? 0x80808080u : 0u;           // threshold 0: no bond at all
+        (void)nth; (void)emask;
 #pragma unroll
         for (int j = 0; j <= ROWS_PER_WARP; ++j) {
             uint32_t gy = y0 + ly0 + j;
@@ -188,16 +196,16 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             philox_stream<STREAM_BOND>(key, (i0 >> 1) + 1u, t, wb);
             uint32_t hn = 0u, vn = 0u;
             if (MODEL == 0) {
-                const uint32_t th = md.thr_potts;
-                const uint32_t dx = cur ^ right, dy = cur ^ nxt;   // byte k zero <=> equal spins
-                hn |= (wa[0] < th && (dx & 0x000000FFu) == 0u) ? 1u : 0u;
-                hn |= (wa[2] < th && (dx & 0x0000FF00u) == 0u) ? 2u : 0u;
-                hn |= (wb[0] < th && (dx & 0x00FF0000u) == 0u) ? 4u : 0u;
-                hn |= (wb[2] < th && (dx & 0xFF000000u) == 0u) ? 8u : 0u;
-                vn |= (wa[1] < th && (dy & 0x000000FFu) == 0u) ? 1u : 0u;
-                vn |= (wa[3] < th && (dy & 0x0000FF00u) == 0u) ? 2u : 0u;
-                vn |= (wb[1] < th && (dy & 0x00FF0000u) == 0u) ? 4u : 0u;
-                vn |= (wb[3] < th && (dy & 0xFF000000u) == 0u) ? 8u : 0u;
+                // [w >= th] is the carry of w + (2^32 - th); add-with-carry shifts it into a nibble (two ALU instructions
+                // per bond instead of compare + select + or); equal spins come from a zero-byte test on the XOR.
+                const uint32_t dx = cur ^ right, dy = cur ^ nxt;   // byte k zero <=> equal spins (bytes < 16)
+                const uint32_t zx = ~(dx + 0x7F7F7F7Fu) & emask, zy = ~(dy + 0x7F7F7F7Fu) & emask;
+                const uint32_t eqh = (zx * 0x00204081u) >> 28, eqv = (zy * 0x00204081u) >> 28;   // bits 7,15,23,31 -> 0..3
+                uint32_t gh = 0u, gv = 0u;
+                ge_shift_in(gh, wb[2], nth); ge_shift_in(gh, wb[0], nth); ge_shift_in(gh, wa[2], nth); ge_shift_in(gh, wa[0], nth);
+                ge_shift_in(gv, wb[3], nth); ge_shift_in(gv, wb[1], nth); ge_shift_in(gv, wa[3], nth); ge_shift_in(gv, wa[1], nth);
+                hn = eqh & ~gh;
+                vn = eqv & ~gv;
             } else {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
