@@ -121,6 +121,11 @@ __device__ __forceinline__ void ge_shift_in(uint32_t &g, uint32_t w, uint32_t nt
 {
     asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(g) : "r"(w), "r"(nth));
 }
+// g = 2 g + [w >= th]: the carry flag after w - th (set when there is no borrow) shifted into g
+__device__ __forceinline__ void ge_sub_shift_in(uint32_t &g, uint32_t w, uint32_t th)
+{
+    asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(g) : "r"(w), "r"(th));
+}
 // K1.  grid = tiles, block = TILE_THREADS.  MODEL 0 = Potts, 1 = clock.
 #ifndef SW_LABEL_MINB
 #define SW_LABEL_MINB 5
@@ -208,13 +213,15 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
                 vn = eqv & ~gv;
             } else {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
+                for (int k = 3; k >= 0; --k) {       // highest site first: every bond shifts its bit in from the right
                     const uint32_t c = (cur >> (8 * k)) & 0xFFu, cr = (right >> (8 * k)) & 0xFFu, cd = (nxt >> (8 * k)) & 0xFFu;
                     const uint32_t wh = (k < 2) ? wa[2 * k] : wb[2 * (k - 2)];
                     const uint32_t wv = (k < 2) ? wa[2 * k + 1] : wb[2 * (k - 2) + 1];
-                    hn |= (wh < s_table[c * q2 + cr]) ? (1u << k) : 0u;
-                    vn |= (wv < s_table[c * q2 + cd]) ? (1u << k) : 0u;
+                    ge_sub_shift_in(hn, wh, s_table[c * q2 + cr]);
+                    ge_sub_shift_in(vn, wv, s_table[c * q2 + cd]);
                 }
+                hn = ~hn & 0xFu;                      // active <=> word < threshold
+                vn = ~vn & 0xFu;
             }
             // gather the nibbles of 8 lanes into one 32-site word: H in the low half, V in the high half
             uint32_t c = hn | (vn << 16);
