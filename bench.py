@@ -133,8 +133,45 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_microbench(args):
+    """Issue-rate probes (sw_microbench): warp-instructions per SM cycle per sub-partition, per opcode and mix.
+    Prints one JSON line per probe and a markdown table (the table is what profiles/ keeps)."""
+    import ctypes
+    import torch
+    from paper_1202_0635_b200 import binding as sw
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --microbench needs a CUDA device")
+    torch.cuda.init()
+    torch.zeros(1, device="cuda")
+    lib = sw.load()
+    warps = [1, 2, 4, 8, 16]
+    rows = []
+    k = 0
+    while True:
+        name = lib.sw_microbench_name(k)
+        if name is None:
+            break
+        rates = []
+        for w in warps:
+            out = (ctypes.c_double * 4)()
+            rc = lib.sw_microbench(k, w, args.mb_iters, out)
+            if rc != 0:
+                raise SystemExit(f"sw_microbench({k}, {w}) failed: {rc}")
+            rates.append(out[0])
+        rows.append((k, name.decode(), rates))
+        print(json.dumps({"probe": k, "name": name.decode(), "warps_per_smsp": warps, "units_per_cycle_per_smsp": rates}), flush=True)
+        k += 1
+    print()
+    print("| probe | " + " | ".join(f"{w} warps/SMSP" for w in warps) + " |")
+    print("|---|" + "---|" * len(warps))
+    for k, name, rates in rows:
+        print(f"| {name} | " + " | ".join(f"{r:.3f}" for r in rates) + " |")
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--microbench", action="store_true", help="run the instruction-issue probes instead of the sweep bench")
+    ap.add_argument("--mb-iters", type=int, default=4000)
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
@@ -145,6 +182,9 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
 
+    if args.microbench:
+        run_microbench(args)
+        return
     if args.impl == "reference":
         run_reference(args)
         return

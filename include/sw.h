@@ -137,6 +137,15 @@ const char *sw_kernel_name(sw_ctx *ctx, int k);
 /* Number of kernel launches this context has enqueued since creation. */
 uint64_t sw_launch_count(sw_ctx *ctx);
 
+/* Instruction-issue probes (measurement infrastructure for the "alu" roofline of DESIGN.md section 6; the sweep never
+ * uses them).  Probe `probe` (0 .. until sw_microbench_name returns NULL) runs `warps_per_smsp` (1..16) warps on every
+ * SM sub-partition of the current device, each executing `iters` loop iterations of 8 independent dependency chains of
+ * one SASS instruction (or a fixed mix, or whole Philox4x32-10 calls).  out (HOST, 4 doubles): [0] = units retired per
+ * SM clock cycle per sub-partition (a unit = one warp-instruction, one pair, or one Philox call, as the name says),
+ * [1] = SM cycles of the slowest CTA, [2] = of the fastest, [3] = units per sub-partition. */
+int sw_microbench(int probe, int warps_per_smsp, int iters, double *out);
+const char *sw_microbench_name(int probe);
+
 /* Thread-local description of the last failure in this thread ("" if none). */
 const char *sw_last_error(void);
 

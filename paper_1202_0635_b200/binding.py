@@ -52,6 +52,8 @@ SYMBOLS = {
     "sw_sweep_profile": (_i, [_vp, _i, _vp, ctypes.POINTER(_i)]),
     "sw_kernel_name": (ctypes.c_char_p, [_vp, _i]),
     "sw_launch_count": (_u64, [_vp]),
+    "sw_microbench": (_i, [_i, _i, _i, _vp]),
+    "sw_microbench_name": (ctypes.c_char_p, [_i]),
     "sw_last_error": (ctypes.c_char_p, []),
 }
 

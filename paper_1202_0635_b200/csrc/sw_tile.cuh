@@ -105,6 +105,24 @@ __device__ __forceinline__ void sunion(uint32_t *lab, uint32_t a, uint32_t b)
     }
 }
 
+// Two A/B switches kept for the record (both measured slower on B200): SW_K1_HILO = mask of the
+// Philox rounds of the labeling kernel computed as IMAD.HI + IMAD (sw_philox.cuh); SW_CLZ_LOOPS = loops over the set
+// bits of a mask take the highest bit first (one FLO per step instead of BREV + FLO).
+#ifndef SW_K1_HILO
+#define SW_K1_HILO 0u
+#endif
+__device__ __forceinline__ uint32_t pop_top(uint32_t &c)
+{
+#ifndef SW_CLZ_LOOPS
+    const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
+    c &= c - 1u;
+#else
+    const uint32_t k = 31u - (uint32_t)__clz((int)c);
+    c ^= 1u << k;
+#endif
+    return k;
+}
+
 // first site (bit position) of the segment that holds bit k; S = mask of segment starts (bit 0 always set)
 __device__ __forceinline__ uint32_t seg_start(uint32_t S, uint32_t k) { return 31u - __clz(S & ((2u << k) - 1u)); }
 
@@ -197,8 +215,8 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             const uint32_t right = (cur >> 8) | (rn << 24);       // byte k = +x neighbour of site k
             const uint32_t i0 = (y0 + ly0 + j) * L + gx;
             uint32_t wa[4], wb[4];
-            philox_stream<STREAM_BOND>(key, i0 >> 1, t, wa);
-            philox_stream<STREAM_BOND>(key, (i0 >> 1) + 1u, t, wb);
+            philox_stream<STREAM_BOND, SW_K1_HILO>(key, i0 >> 1, t, wa);
+            philox_stream<STREAM_BOND, SW_K1_HILO>(key, (i0 >> 1) + 1u, t, wb);
             uint32_t hn = 0u, vn = 0u;
             if (MODEL == 0) {
                 // [w >= th] is the carry of w + (2^32 - th); add-with-carry shifts it into a nibble (two ALU instructions
@@ -296,16 +314,16 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
     }
     {
         uint32_t *el = s_edge[warp];
-        for (uint32_t c = cs; c; c &= c - 1u) {
-            const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
+        for (uint32_t c = cs; c;) {
+            const uint32_t k = pop_top(c);
             s_lab[sb + k] = sb + k;
         }
-        for (uint32_t f = first; f; f &= f - 1u) {
-            const uint32_t k = (uint32_t)__ffs((int)f) - 1u;
+        for (uint32_t f = first; f;) {
+            const uint32_t k = pop_top(f);
             s_lab[sb + seg_start(S, k)] = sbu + seg_start(Sa, k);
         }
-        for (uint32_t xr = X; xr; xr &= xr - 1u) {
-            const uint32_t k = (uint32_t)__ffs((int)xr) - 1u;
+        for (uint32_t xr = X; xr;) {
+            const uint32_t k = pop_top(xr);
             if (epos < (uint32_t)EDGE_CAP) el[epos] = (sb + seg_start(S, k)) | ((sbu + seg_start(Sa, k)) << 16);
             ++epos;
         }
@@ -382,8 +400,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             // rare: the list overflowed; this thread unions its unlisted edges itself
             uint32_t slot = epos0, Xr = X;
             while (Xr) {
-                const uint32_t k = (uint32_t)__ffs((int)Xr) - 1u;
-                Xr &= Xr - 1u;
+                const uint32_t k = pop_top(Xr);
                 if (slot >= (uint32_t)EDGE_CAP) sunion(s_lab, sb + seg_start(S, k), sbu + seg_start(Sa, k));
                 ++slot;
             }
@@ -456,13 +473,13 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
                 ax |= ((z * 0x00204081u) >> 28) << (4 * j);          // bits 7, 15, 23, 31 -> one nibble
             }
             cand &= ~ax;
-            for (; ax; ax &= ax - 1u) {
-                const uint32_t k = (uint32_t)__ffs((int)ax) - 1u;
+            while (ax) {
+                const uint32_t k = pop_top(ax);
                 vl[sb + k] = (sb + k) | ((fuse ? (uint32_t)DEC_BASE : sb + k) << 16);
             }
         }
-        for (uint32_t c = cand; c; c &= c - 1u) {
-            const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
+        for (uint32_t c = cand; c;) {
+            const uint32_t k = pop_top(c);
             const uint32_t v = vl[sb + k];
             if ((v & LMASK) == sb + k) rall |= 1u << k;
         }
@@ -480,8 +497,8 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
         const bool listed = total <= (uint32_t)RCAP;
         if (listed) {
             uint32_t at = incl - n;
-            for (uint32_t rr = rall; rr; rr &= rr - 1u) {
-                const uint32_t k = (uint32_t)__ffs((int)rr) - 1u;
+            for (uint32_t rr = rall; rr;) {
+                const uint32_t k = pop_top(rr);
                 rl[at++] = (uint16_t)vl[sb + k];
             }
             __syncwarp();
@@ -494,8 +511,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             if (listed) {
                 e = rl[i];
             } else {
-                const uint32_t k = (uint32_t)__ffs((int)mine) - 1u;
-                mine &= mine - 1u;
+                const uint32_t k = pop_top(mine);
                 e = vl[sb + k] & 0xFFFFu;
             }
             const uint32_t sp = e & LMASK;
@@ -509,7 +525,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
                 out = LOPEN | pos;
             } else if (fuse) {
                 uint32_t w[4];
-                philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
+                philox_stream<STREAM_CLUSTER, SW_K1_HILO>(key, r >> 2, t, w);
                 const uint32_t wsel = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
                 out = (uint32_t)DEC_BASE + (MODEL == 0 ? mulhi_q(wsel, (uint32_t)md.q) : (wsel >> 31));
             }
@@ -532,9 +548,14 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ sp
             uint32_t rem = 0u;
             while (todo) {
                 // the lowest and the highest run still to do (the same run when one is left: harmless repeat)
+#ifndef SW_CLZ_LOOPS
                 const uint32_t k0 = (uint32_t)__ffs((int)todo) - 1u, k1 = 31u - (uint32_t)__clz((int)todo);
                 todo &= todo - 1u;
                 todo &= ~(1u << k1);
+#else
+                const uint32_t k1 = pop_top(todo);
+                const uint32_t k0 = todo ? pop_top(todo) : k1;
+#endif
                 uint32_t x0 = vl[sb + k0], x1 = vl[sb + k1];
                 x0 = vl[x0 & LMASK]; x1 = vl[x1 & LMASK];
                 const uint32_t y0r = vl[x0 & LMASK], y1r = vl[x1 & LMASK];
