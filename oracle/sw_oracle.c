@@ -11,7 +11,8 @@
  * Where the paper is silent the readings of DESIGN.md section 3 (R1..R15) are used; each is
  * cited at its point of use.  Parity status: every function below is pinned by tests/ (Philox
  * known answers, high-precision thresholds, brute-force flood fill, exact enumeration of the
- * Boltzmann distribution on small tori, Kaufman/Onsager energy; oracle_correlation: tests/test_oracle_corr_pins.py)
+ * Boltzmann distribution on small tori, Kaufman/Onsager energy; oracle_correlation: tests/test_oracle_corr_pins.py;
+ * the derived doubles oracle_potts_energy .. oracle_ratio_R: tests/test_oracle_derived_pins.py)
  * -- nothing is "parity unpinned".
  *
  * Conventions: N = L*L, site i = y*L + x (x fastest).  Each site owns two bonds:
@@ -297,6 +298,84 @@ void oracle_correlation(int L, int q, const uint8_t *spins, int r, int64_t *corr
             corr_hist[((s - sy) % q + q) % q] += 1;
         }
     }
+}
+
+/* ------------------------------------------------------------------------------------------- */
+/* Derived doubles (R11, R15): what the paper plots, computed from the integer histograms in a    */
+/* fixed order (sums run over d or k ascending, left to right, in double).                        */
+/* ------------------------------------------------------------------------------------------- */
+#define ORACLE_PI 3.14159265358979323846
+
+/* Potts energy of eq.(1), in units of J: every owned bond with unequal spins costs 1. */
+double oracle_potts_energy(int L, const int64_t *bond_hist)
+{
+    return (double)(2 * (int64_t)L * (int64_t)L - bond_hist[0]);
+}
+
+/* Eq.(3): M^2 = (q sum_k n[k]^2 - N^2) / (q - 1).  The numerator is an exact integer
+ * (< 2^63 for N <= 2^28, q <= 16); one division in double. */
+double oracle_potts_m2(int q, const int64_t *state_hist)
+{
+    int64_t N = 0, acc = 0;
+    for (int k = 0; k < q; ++k) { N += state_hist[k]; acc += state_hist[k] * state_hist[k]; }
+    return (double)((int64_t)q * acc - N * N) / (double)(q - 1);
+}
+
+/* Clock energy of eq.(4), in units of J: - sum over owned bonds of cos(theta_i - theta_j). */
+double oracle_clock_energy(int q, const int64_t *bond_hist)
+{
+    double e = 0.0;
+    for (int d = 0; d < q; ++d) e += (double)bond_hist[d] * cos(2.0 * ORACLE_PI * (double)d / (double)q);
+    return -e;
+}
+
+/* |M| of the clock model: length of the vector sum of the planar unit spins. */
+double oracle_clock_m(int q, const int64_t *state_hist)
+{
+    double mx = 0.0, my = 0.0;
+    for (int k = 0; k < q; ++k) {
+        mx += (double)state_hist[k] * cos(2.0 * ORACLE_PI * (double)k / (double)q);
+        my += (double)state_hist[k] * sin(2.0 * ORACLE_PI * (double)k / (double)q);
+    }
+    return hypot(mx, my);
+}
+
+/* Eq.(5), for one configuration: G(r) = (1/pairs) sum over the counted pairs of S_i . S_{i+r}
+ * = (1/pairs) sum_d corr_hist[d] cos(2 pi d / q)  (R15). */
+double oracle_g(int q, const int64_t *corr_hist)
+{
+    double g = 0.0;
+    int64_t pairs = 0;
+    for (int d = 0; d < q; ++d) {
+        g += (double)corr_hist[d] * cos(2.0 * ORACLE_PI * (double)d / (double)q);
+        pairs += corr_hist[d];
+    }
+    return g / (double)pairs;
+}
+
+/* Eq.(2): U = <M^4> / <M^2>^2 over a recorded series of n state histograms (rows of q), M^2 of
+ * every row by eq.(3), averages accumulated row by row. */
+double oracle_moment_ratio(int n, int q, const int64_t *state_hist_rows)
+{
+    double s2 = 0.0, s4 = 0.0;
+    for (int k = 0; k < n; ++k) {
+        double m2 = oracle_potts_m2(q, state_hist_rows + (size_t)k * q);
+        s2 += m2;
+        s4 += m2 * m2;
+    }
+    return (s4 / (double)n) / ((s2 / (double)n) * (s2 / (double)n));
+}
+
+/* Eq.(6): R = <G(L/2)> / <G(L/4)>, the averages of eq.(5) over a recorded series of n
+ * correlation histograms at the two distances (rows of q). */
+double oracle_ratio_R(int n, int q, const int64_t *corr_half_rows, const int64_t *corr_quarter_rows)
+{
+    double gh = 0.0, gq = 0.0;
+    for (int k = 0; k < n; ++k) {
+        gh += oracle_g(q, corr_half_rows + (size_t)k * q);
+        gq += oracle_g(q, corr_quarter_rows + (size_t)k * q);
+    }
+    return (gh / (double)n) / (gq / (double)n);
 }
 
 /* n sweeps t0 .. t0+n-1.  If bond_rec/state_rec are non-NULL, row k (q entries each) receives

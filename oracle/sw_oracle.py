@@ -78,6 +78,13 @@ def lib() -> ctypes.CDLL:
         L.oracle_run.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                  ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int, _u8p, _i64p, _i64p]
         L.oracle_run.restype = ctypes.c_int
+        for name, args in (("oracle_potts_energy", [ctypes.c_int, _i64p]), ("oracle_potts_m2", [ctypes.c_int, _i64p]),
+                           ("oracle_clock_energy", [ctypes.c_int, _i64p]), ("oracle_clock_m", [ctypes.c_int, _i64p]),
+                           ("oracle_g", [ctypes.c_int, _i64p]), ("oracle_moment_ratio", [ctypes.c_int, ctypes.c_int, _i64p]),
+                           ("oracle_ratio_R", [ctypes.c_int, ctypes.c_int, _i64p, _i64p])):
+            fn = getattr(L, name)
+            fn.argtypes = args
+            fn.restype = ctypes.c_double
         _lib = L
     return _lib
 
@@ -175,6 +182,44 @@ def correlation(L, q, spins, r):
     ch = np.zeros(q, dtype=np.int64)
     lib().oracle_correlation(L, q, _p(s, _u8p), int(r), _p(ch, _i64p))
     return ch
+
+
+def _i64(a, shape=None) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.int64)
+    if shape is not None:
+        a = a.reshape(shape)
+    return a
+
+
+def potts_energy(L, bond_hist) -> float:
+    return float(lib().oracle_potts_energy(L, _p(_i64(bond_hist), _i64p)))
+
+
+def potts_m2(q, state_hist) -> float:
+    return float(lib().oracle_potts_m2(q, _p(_i64(state_hist), _i64p)))
+
+
+def clock_energy(q, bond_hist) -> float:
+    return float(lib().oracle_clock_energy(q, _p(_i64(bond_hist), _i64p)))
+
+
+def clock_m(q, state_hist) -> float:
+    return float(lib().oracle_clock_m(q, _p(_i64(state_hist), _i64p)))
+
+
+def g(q, corr_hist) -> float:
+    return float(lib().oracle_g(q, _p(_i64(corr_hist), _i64p)))
+
+
+def moment_ratio(q, state_hist_rows) -> float:
+    rows = _i64(state_hist_rows, (-1, q))
+    return float(lib().oracle_moment_ratio(rows.shape[0], q, _p(rows, _i64p)))
+
+
+def ratio_R(q, corr_half_rows, corr_quarter_rows) -> float:
+    a, b = _i64(corr_half_rows, (-1, q)), _i64(corr_quarter_rows, (-1, q))
+    assert a.shape == b.shape
+    return float(lib().oracle_ratio_R(a.shape[0], q, _p(a, _i64p), _p(b, _i64p)))
 
 
 def run(L, q, model, T, seed, t0, n, spins, record=False):
