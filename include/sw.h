@@ -80,7 +80,7 @@ int sw_sweep_record(sw_ctx *ctx, int n, int64_t *bond_hist_out, int64_t *state_h
 
 /* Observables of the current configuration, HOST outputs of q int64 each (R11):
  * bond_hist[d] = #{owned bonds with (S_i - S_nbr) mod q == d};  state_hist[k] = #{S_i == k}.
- * Potts energy E/J = 2*L*L - bond_hist[0]; M^2 from state_hist by eq.(3). */
+ * Derived doubles: sw_derive_* below. */
 int sw_observables(sw_ctx *ctx, int64_t *bond_hist, int64_t *state_hist);
 
 /* NEXT-1 of the scope table: the correlation function of PAPER.md eq.(5) at distance r, as an integer histogram
@@ -92,6 +92,24 @@ int sw_observables(sw_ctx *ctx, int64_t *bond_hist, int64_t *state_hist);
 int sw_correlation(sw_ctx *ctx, int r, int64_t *corr_hist);
 int sw_sweep_record_corr(sw_ctx *ctx, int n, int r1, int r2, int64_t *bond_hist_out, int64_t *state_hist_out,
                          int64_t *corr1_out, int64_t *corr2_out);
+
+/* The doubles the paper plots, derived from the integer histograms above (HOST inputs; plain host arithmetic in a
+ * fixed order -- sums run over d or k ascending, left to right, in double; R11, R15).  NaN on invalid
+ * arguments (NULL, q outside 2..16, n < 1).
+ *   sw_derive_potts_energy  E/J of eq.(1) = 2*L*L - bond_hist[0]
+ *   sw_derive_potts_m2      M^2 of eq.(3) = (q sum_k n[k]^2 - N^2) / (q - 1), integer numerator
+ *   sw_derive_clock_energy  E/J of eq.(4) = - sum_d bond_hist[d] cos(2 pi d / q)
+ *   sw_derive_clock_m       |sum_i S_i| of the planar unit spins, from state_hist
+ *   sw_derive_g             G(r) of eq.(5) of one configuration = sum_d corr_hist[d] cos(2 pi d / q) / pairs
+ *   sw_derive_moment_ratio  U = <M^4> / <M^2>^2 of eq.(2) over n recorded rows of q state counts
+ *   sw_derive_ratio_R       R = <G(L/2)> / <G(L/4)> of eq.(6) over n recorded rows of q pair counts each */
+double sw_derive_potts_energy(int L, const int64_t *bond_hist);
+double sw_derive_potts_m2(int q, const int64_t *state_hist);
+double sw_derive_clock_energy(int q, const int64_t *bond_hist);
+double sw_derive_clock_m(int q, const int64_t *state_hist);
+double sw_derive_g(int q, const int64_t *corr_hist);
+double sw_derive_moment_ratio(int n, int q, const int64_t *state_hist_rows);
+double sw_derive_ratio_R(int n, int q, const int64_t *corr_half_rows, const int64_t *corr_quarter_rows);
 
 /* Copy the configuration to / from HOST memory (L*L bytes, row-major, values 0..q-1).
  * sw_set_spins also sets the absolute sweep index (resume / oracle hand-off); values >= q are
@@ -145,6 +163,11 @@ uint64_t sw_launch_count(sw_ctx *ctx);
  * [1] = SM cycles of the slowest CTA, [2] = of the fastest, [3] = units per sub-partition. */
 int sw_microbench(int probe, int warps_per_smsp, int iters, double *out);
 const char *sw_microbench_name(int probe);
+
+/* Device self-test of the kernels' carry-flag threshold compares ([word >= threshold] shifted in through add.cc / sub.cc
+ * + addc) against the plain comparison over edge values on the current device: SW_OK, or SW_ERR_UNSUPPORTED if the
+ * toolchain's carry convention differs from the one the kernels were written for (every clock bond would flip). */
+int sw_selftest(void);
 
 /* Thread-local description of the last failure in this thread ("" if none). */
 const char *sw_last_error(void);

@@ -52,8 +52,16 @@ SYMBOLS = {
     "sw_sweep_profile": (_i, [_vp, _i, _vp, ctypes.POINTER(_i)]),
     "sw_kernel_name": (ctypes.c_char_p, [_vp, _i]),
     "sw_launch_count": (_u64, [_vp]),
+    "sw_derive_potts_energy": (_d, [_i, _vp]),
+    "sw_derive_potts_m2": (_d, [_i, _vp]),
+    "sw_derive_clock_energy": (_d, [_i, _vp]),
+    "sw_derive_clock_m": (_d, [_i, _vp]),
+    "sw_derive_g": (_d, [_i, _vp]),
+    "sw_derive_moment_ratio": (_d, [_i, _i, _vp]),
+    "sw_derive_ratio_R": (_d, [_i, _i, _vp, _vp]),
     "sw_microbench": (_i, [_i, _i, _i, _vp]),
     "sw_microbench_name": (ctypes.c_char_p, [_i]),
+    "sw_selftest": (_i, []),
     "sw_last_error": (ctypes.c_char_p, []),
 }
 
@@ -240,101 +248,38 @@ class Lattice:
         return int(self._lib.sw_launch_count(self._h))
 
 
-# Derived doubles (R11): fixed summation order, computed by the caller from the integers.
+# Derived doubles (R11, R15): computed by libsw.so (sw_derive_*), marshalled here.
+def _i64(a, q=None) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.int64)
+    return a if q is None else a.reshape(-1, q)
+
+
 def potts_energy(L: int, bond_hist) -> float:
-    return float(2 * L * L - int(bond_hist[0]))
+    return float(load().sw_derive_potts_energy(L, _i64(bond_hist).ctypes.data))
 
 
 def potts_m2(q: int, state_hist) -> float:
-    """Eq.(3): M^2 = (q sum_k n[k]^2 - N^2) / (q - 1)."""
-    n = [int(x) for x in state_hist]
-    N = sum(n)
-    acc = 0
-    for k in range(q):
-        acc += n[k] * n[k]
-    return float(q * acc - N * N) / float(q - 1)
+    return float(load().sw_derive_potts_m2(q, _i64(state_hist).ctypes.data))
 
 
 def clock_energy(q: int, bond_hist) -> float:
-    import math
-    e = 0.0
-    for d in range(q):
-        e += float(int(bond_hist[d])) * math.cos(2.0 * math.pi * d / q)
-    return -e
+    return float(load().sw_derive_clock_energy(q, _i64(bond_hist).ctypes.data))
 
 
-def clock_magnetisation(q: int, state_hist) -> float:
-    import math
-    mx = 0.0
-    my = 0.0
-    for k in range(q):
-        mx += float(int(state_hist[k])) * math.cos(2.0 * math.pi * k / q)
-        my += float(int(state_hist[k])) * math.sin(2.0 * math.pi * k / q)
-    return math.hypot(mx, my)
+def clock_m(q: int, state_hist) -> float:
+    return float(load().sw_derive_clock_m(q, _i64(state_hist).ctypes.data))
 
 
-def correlation_g(q: int, corr_hist) -> float:
-    """G(r) of PAPER.md eq.(5) from the integer histogram: (1 / 2N) sum_d corr_hist[d] cos(2 pi d / q), d ascending."""
-    import math
-    g = 0.0
-    n = 0
-    for d in range(q):
-        g += float(int(corr_hist[d])) * math.cos(2.0 * math.pi * d / q)
-        n += int(corr_hist[d])
-    return g / float(n)
+def g(q: int, corr_hist) -> float:
+    return float(load().sw_derive_g(q, _i64(corr_hist).ctypes.data))
 
 
-def moment_ratio(m2_series) -> float:
-    """U of PAPER.md eq.(2): <M^4> / <M^2>^2 over a series of M^2 values (eq.(3)), accumulated left to right."""
-    s2 = 0.0
-    s4 = 0.0
-    for m2 in m2_series:
-        s2 += float(m2)
-        s4 += float(m2) * float(m2)
-    k = float(len(m2_series))
-    return (s4 / k) / ((s2 / k) * (s2 / k))
+def moment_ratio(q: int, state_hist_rows) -> float:
+    rows = _i64(state_hist_rows, q)
+    return float(load().sw_derive_moment_ratio(rows.shape[0], q, rows.ctypes.data))
 
 
-# The C names, as plain functions over a Lattice (same names as include/sw.h).
-def sw_create(L, q, model, T, seed) -> Lattice:
-    return Lattice(L, q, model, T, seed)
-
-
-def sw_destroy(ctx: Lattice):
-    ctx.close()
-
-
-def sw_sweep(ctx: Lattice, n: int):
-    ctx.sweep(n)
-
-
-def sw_sweep_record(ctx: Lattice, n: int):
-    return ctx.sweep_record(n)
-
-
-def sw_get_spins(ctx: Lattice, out=None):
-    return ctx.get_spins(out)
-
-
-def sw_set_spins(ctx: Lattice, spins, sweep_index: int = 0):
-    ctx.set_spins(spins, sweep_index)
-
-
-def sw_observables(ctx: Lattice):
-    return ctx.observables()
-
-
-def sw_get_thresholds(ctx: Lattice):
-    return ctx.get_thresholds()
-
-
-def sw_get_labels(ctx: Lattice):
-    return ctx.get_labels()
-
-
-def sw_correlation(ctx: Lattice, r: int):
-    return ctx.correlation(r)
-
-
-def sw_sweep_record_corr(ctx: Lattice, n: int, r1: int, r2: int):
-    return ctx.sweep_record_corr(n, r1, r2)
+def ratio_R(q: int, corr_half_rows, corr_quarter_rows) -> float:
+    a, b = _i64(corr_half_rows, q), _i64(corr_quarter_rows, q)
+    assert a.shape == b.shape
+    return float(load().sw_derive_ratio_R(a.shape[0], q, a.ctypes.data, b.ctypes.data))

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <utility>
@@ -81,6 +82,7 @@ struct sw_ctx {
     uint64_t seed = 0, t = 0;
     size_t N = 0;
     cudaStream_t stream = nullptr;
+    int device = 0, sms = 148;      // the device the workspace and stream belong to; its SM count (grid sizing)
     bool own_stream = false, own_ws = false;
     char *ws = nullptr;
     Carve cv{};
@@ -101,6 +103,18 @@ struct sw_ctx {
 };
 
 namespace {
+
+// A context belongs to the device that was current when it was created: every entry point makes that device current
+// for its own duration and restores the caller's on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const sw_ctx *c)
+    {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 uint32_t thr_from_p(double p)
 {
@@ -150,6 +164,7 @@ int generic_sweep(sw_ctx *c, uint32_t t, cudaEvent_t *ev)
     sw::k_flip<<<blocks_for(N, bs), bs, 0, c->stream>>>(c->md, c->key, t, c->labels, c->spins);
     if (ev) cudaEventRecord(ev[5], c->stream);
     c->launches += 5;
+    CU_TRY(cudaPeekAtLastError());
     return SW_OK;
 }
 
@@ -176,12 +191,14 @@ int launch_observables(sw_ctx *c, unsigned long long *dst, bool zero = true)   /
 {
     if (zero) CU_TRY(cudaMemsetAsync(dst, 0, 8 * OBS_WORDS, c->stream));
     const size_t work = (c->L % 16 == 0) ? c->N / 16 : c->N;
-    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 4));
+    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, (size_t)c->sms * 4));
     const uint8_t *sp = c->spins;
-    if (c->q <= 2) sw::launch_pdl(sw::k_observables<2>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
-    else if (c->q <= 4) sw::launch_pdl(sw::k_observables<4>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
-    else if (c->q <= 8) sw::launch_pdl(sw::k_observables<8>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
-    else sw::launch_pdl(sw::k_observables<16>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
+    cudaError_t e;
+    if (c->q <= 2) e = sw::launch_pdl(sw::k_observables<2>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
+    else if (c->q <= 4) e = sw::launch_pdl(sw::k_observables<4>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
+    else if (c->q <= 8) e = sw::launch_pdl(sw::k_observables<8>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
+    else e = sw::launch_pdl(sw::k_observables<16>, grid, sw::HIST_THREADS, c->stream, c->md, sp, dst);
+    CU_TRY(e);
     c->launches += 1;
     return SW_OK;
 }
@@ -189,13 +206,15 @@ int launch_observables(sw_ctx *c, unsigned long long *dst, bool zero = true)   /
 int launch_correlation(sw_ctx *c, int r, unsigned long long *dst)   // dst: 16 zeroed words
 {
     const size_t work = (c->L % 16 == 0 && r % 4 == 0) ? c->N / 16 : (c->L % 4 == 0) ? c->N / 4 : c->N;
-    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, 148 * 4));
+    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, (size_t)c->sms * 4));
     const uint8_t *sp = c->spins;
     const uint32_t ur = (uint32_t)r;
-    if (c->q <= 2) sw::launch_pdl(sw::k_correlation<2>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
-    else if (c->q <= 4) sw::launch_pdl(sw::k_correlation<4>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
-    else if (c->q <= 8) sw::launch_pdl(sw::k_correlation<8>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
-    else sw::launch_pdl(sw::k_correlation<16>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
+    cudaError_t e;
+    if (c->q <= 2) e = sw::launch_pdl(sw::k_correlation<2>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
+    else if (c->q <= 4) e = sw::launch_pdl(sw::k_correlation<4>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
+    else if (c->q <= 8) e = sw::launch_pdl(sw::k_correlation<8>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
+    else e = sw::launch_pdl(sw::k_correlation<16>, grid, sw::HIST_THREADS, c->stream, c->md, sp, ur, dst);
+    CU_TRY(e);
     c->launches += 1;
     return SW_OK;
 }
@@ -215,8 +234,14 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
     }
     sw_ctx *c = new (std::nothrow) sw_ctx();
     if (!c) { fail(SW_ERR_NOMEM, "sw_create: out of host memory"); return nullptr; }
+    if (const char *ds = std::getenv("SW_DUMMY_SMEM")) sw::g_pdl_dynamic_smem = (unsigned)std::atoi(ds);
     c->L = L; c->q = q; c->model = model; c->T = T; c->seed = seed; c->t = 0;
     c->N = (size_t)L * (size_t)L;
+    if (cudaGetDevice(&c->device) != cudaSuccess || cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) {
+        fail(SW_ERR_CUDA, "sw_create: cannot query the current device: %s", cudaGetErrorString(cudaGetLastError()));
+        delete c;
+        return nullptr;
+    }
     c->cv = carve(L, q);
     if (own) {
         cudaError_t e = cudaMalloc((void **)&c->ws, c->cv.total);
@@ -304,6 +329,7 @@ sw_ctx *sw_create_in(int L, int q, int model, double T, uint64_t seed, void *d_w
 void sw_destroy(sw_ctx *c)
 {
     if (!c) return;
+    DeviceGuard guard(c);
     if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
     if (c->own_ws && c->ws) cudaFree(c->ws);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
@@ -313,6 +339,7 @@ void sw_destroy(sw_ctx *c)
 int sw_sweep_async(sw_ctx *c, int n)
 {
     if (!c || n < 0) return fail(SW_ERR_ARG, "sw_sweep: NULL context or n < 0");
+    DeviceGuard guard(c);
     if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep: sweep index would exceed 2^32-1");
     for (int k = 0; k < n; ++k) {
         int rc = one_sweep(c);
@@ -325,6 +352,7 @@ int sw_sweep_async(sw_ctx *c, int n)
 int sw_sync(sw_ctx *c)
 {
     if (!c) return fail(SW_ERR_ARG, "sw_sync: NULL context");
+    DeviceGuard guard(c);
     CU_TRY(cudaStreamSynchronize(c->stream));
     return SW_OK;
 }
@@ -351,8 +379,9 @@ int record_impl(sw_ctx *c, int n, int r1, int r2, int64_t *bond_out, int64_t *st
             int rc = launch_observables(c, row, false);
             if (rc != SW_OK) return rc;
             if (r1 >= 0) {
-                launch_correlation(c, r1, row + 32);
-                launch_correlation(c, r2, row + 48);
+                rc = launch_correlation(c, r1, row + 32);
+                if (rc == SW_OK) rc = launch_correlation(c, r2, row + 48);
+                if (rc != SW_OK) return rc;
             }
             rc = one_sweep(c);
             if (rc != SW_OK) return rc;
@@ -379,6 +408,7 @@ int record_impl(sw_ctx *c, int n, int r1, int r2, int64_t *bond_out, int64_t *st
 int sw_sweep_record(sw_ctx *c, int n, int64_t *bond_out, int64_t *state_out)
 {
     if (!c || n < 0 || !bond_out || !state_out) return fail(SW_ERR_ARG, "sw_sweep_record: bad arguments");
+    DeviceGuard guard(c);
     if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_record: sweep index would exceed 2^32-1");
     return record_impl(c, n, -1, -1, bond_out, state_out, nullptr, nullptr);
 }
@@ -388,6 +418,7 @@ int sw_sweep_record_corr(sw_ctx *c, int n, int r1, int r2, int64_t *bond_out, in
 {
     if (!c || n < 0 || !bond_out || !state_out || !corr1_out || !corr2_out || r1 < 0 || r2 < 0 || r1 >= c->L || r2 >= c->L)
         return fail(SW_ERR_ARG, "sw_sweep_record_corr: bad arguments (need 0 <= r1, r2 < L and non-NULL outputs)");
+    DeviceGuard guard(c);
     if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_record_corr: sweep index would exceed 2^32-1");
     return record_impl(c, n, r1, r2, bond_out, state_out, corr1_out, corr2_out);
 }
@@ -395,8 +426,10 @@ int sw_sweep_record_corr(sw_ctx *c, int n, int r1, int r2, int64_t *bond_out, in
 int sw_correlation(sw_ctx *c, int r, int64_t *corr_hist)
 {
     if (!c || !corr_hist || r < 0 || r >= c->L) return fail(SW_ERR_ARG, "sw_correlation: need 0 <= r < L and a non-NULL output");
+    DeviceGuard guard(c);
     CU_TRY(cudaMemsetAsync(c->obs, 0, 8 * OBS_WORDS, c->stream));
-    launch_correlation(c, r, c->obs + 32);
+    int rc = launch_correlation(c, r, c->obs + 32);
+    if (rc != SW_OK) return rc;
     CU_TRY(cudaGetLastError());
     unsigned long long host[16];
     CU_TRY(cudaMemcpyAsync(host, c->obs + 32, sizeof(host), cudaMemcpyDeviceToHost, c->stream));
@@ -408,6 +441,7 @@ int sw_correlation(sw_ctx *c, int r, int64_t *corr_hist)
 int sw_observables(sw_ctx *c, int64_t *bond_hist, int64_t *state_hist)
 {
     if (!c || !bond_hist || !state_hist) return fail(SW_ERR_ARG, "sw_observables: NULL argument");
+    DeviceGuard guard(c);
     int rc = launch_observables(c, c->obs);
     if (rc != SW_OK) return rc;
     CU_TRY(cudaGetLastError());
@@ -424,6 +458,7 @@ int sw_observables(sw_ctx *c, int64_t *bond_hist, int64_t *state_hist)
 int sw_get_spins(sw_ctx *c, uint8_t *host_out)
 {
     if (!c || !host_out) return fail(SW_ERR_ARG, "sw_get_spins: NULL argument");
+    DeviceGuard guard(c);
     CU_TRY(cudaMemcpyAsync(host_out, c->spins, c->N, cudaMemcpyDeviceToHost, c->stream));
     CU_TRY(cudaStreamSynchronize(c->stream));
     return SW_OK;
@@ -432,6 +467,7 @@ int sw_get_spins(sw_ctx *c, uint8_t *host_out)
 int sw_set_spins(sw_ctx *c, const uint8_t *host_in, uint64_t sweep_index)
 {
     if (!c || !host_in) return fail(SW_ERR_ARG, "sw_set_spins: NULL argument");
+    DeviceGuard guard(c);
     if (sweep_index > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_set_spins: sweep index must fit 32 bits");
     // Stage in the bond scratch buffer, validate on the device, then commit.
     CU_TRY(cudaMemcpyAsync(c->bonds, host_in, c->N, cudaMemcpyHostToDevice, c->stream));
@@ -463,18 +499,24 @@ int sw_get_thresholds(sw_ctx *c, uint32_t *out, int *count)
 int sw_get_labels(sw_ctx *c, int32_t *host_out)
 {
     if (!c || !host_out) return fail(SW_ERR_ARG, "sw_get_labels: NULL argument");
+    DeviceGuard guard(c);
     if (!c->have_labels) return fail(SW_ERR_ARG, "sw_get_labels: no sweep has been executed on this configuration");
     if (c->last_algo == SW_ALGO_TILED) {
         // The tiled sweep fuses the decisions of tile-local clusters into its labels, so the canonical roots are
         // rebuilt from the sweep's input (still in the other ping-pong buffer) and its bonds (sweep index t - 1).
-        int32_t *tmp = nullptr;
-        CU_TRY(cudaMalloc((void **)&tmp, 4 * c->N));
-        int rc = sw::tiled_relabel(c->tiled, c->md, c->key, (uint32_t)(c->t - 1), c->spins_alt, (unsigned long long *)c->labels, tmp, c->stream,
-                                   &c->launches);
-        cudaError_t e = rc == 0 ? cudaMemcpyAsync(host_out, tmp, 4 * c->N, cudaMemcpyDeviceToHost, c->stream) : cudaErrorUnknown;
-        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-        cudaFree(tmp);
-        if (e != cudaSuccess) return fail(SW_ERR_CUDA, "sw_get_labels: resolve failed: %s", cudaGetErrorString(cudaGetLastError()));
+        // No allocation: the union-find nodes take the first N/2 bytes of the 4N-byte label array, the resolved labels
+        // are staged behind them, half of the lattice (2N bytes) at a time.
+        unsigned long long *parent = (unsigned long long *)c->labels;
+        int32_t *stage = c->labels + c->N / 4;           // byte offset N: past the N/2 bytes of nodes, 1024-aligned
+        if (sw::tiled_relabel(c->tiled, c->md, c->key, (uint32_t)(c->t - 1), c->spins_alt, parent, c->stream, &c->launches) != 0)
+            return fail(SW_ERR_CUDA, "sw_get_labels: relabel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        const uint32_t half = (uint32_t)(c->N / 2);
+        for (uint32_t part = 0; part < 2; ++part) {
+            if (sw::tiled_resolve_chunk(c->tiled, c->md, parent, part * half, half, stage, c->stream, &c->launches) != 0)
+                return fail(SW_ERR_CUDA, "sw_get_labels: resolve launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+            CU_TRY(cudaMemcpyAsync(host_out + (size_t)part * half, stage, 4 * (size_t)half, cudaMemcpyDeviceToHost, c->stream));
+            CU_TRY(cudaStreamSynchronize(c->stream));
+        }
         return SW_OK;
     }
     CU_TRY(cudaGetLastError());
@@ -486,6 +528,7 @@ int sw_get_labels(sw_ctx *c, int32_t *host_out)
 int sw_debug_bonds(sw_ctx *c, uint8_t *host_out)
 {
     if (!c || !host_out) return fail(SW_ERR_ARG, "sw_debug_bonds: NULL argument");
+    DeviceGuard guard(c);
     sw::k_bonds<<<blocks_for((c->N + 1) / 2, 256), 256, 0, c->stream>>>(c->md, c->key, (uint32_t)c->t, c->spins, c->bonds);
     c->launches += 1;
     CU_TRY(cudaGetLastError());
@@ -517,6 +560,7 @@ int sw_enable_stats(sw_ctx *c, int on)
 int sw_stats(sw_ctx *c, double *out4)
 {
     if (!c || !out4) return fail(SW_ERR_ARG, "sw_stats: NULL argument");
+    DeviceGuard guard(c);
     unsigned long long h[SW_NUM_STATS];
     CU_TRY(cudaMemcpyAsync(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CU_TRY(cudaStreamSynchronize(c->stream));
@@ -528,6 +572,7 @@ int sw_stats(sw_ctx *c, double *out4)
 int sw_sweep_profile(sw_ctx *c, int n, double *ms_out, int *n_kernels)
 {
     if (!c || n < 0 || !ms_out || !n_kernels) return fail(SW_ERR_ARG, "sw_sweep_profile: bad arguments");
+    DeviceGuard guard(c);
     if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_profile: sweep index would exceed 2^32-1");
     const int nk = (c->algo == SW_ALGO_TILED) ? sw::TILED_NUM_KERNELS : 5;
     cudaEvent_t ev[SW_MAX_KERNELS + 1];
@@ -557,6 +602,34 @@ const char *sw_kernel_name(sw_ctx *c, int k)
 }
 
 uint64_t sw_launch_count(sw_ctx *c) { return c ? c->launches : 0; }
+
+int sw_selftest(void)
+{
+    static const uint32_t base[] = { 0u, 1u, 2u, 0x7FFFFFFFu, 0x80000000u, 0x80000001u, 0x95F61998u, 0xAAAAAAAAu, 0xFFFFFFFEu, 0xFFFFFFFFu };
+    std::vector<uint32_t> v(base, base + sizeof(base) / sizeof(base[0]));
+    for (uint32_t k = 0; k < 54; ++k) v.push_back(0x9E3779B9u * (k + 1u) + (k << 27));
+    for (size_t k = 0, n0 = v.size(); k < n0; ++k) { v.push_back(v[k] + 1u); v.push_back(v[k] - 1u); }
+    const int n = (int)v.size();
+    uint32_t *d_v = nullptr;
+    int *d_bad = nullptr;
+    CU_TRY(cudaMalloc((void **)&d_v, 4 * (size_t)n));
+    cudaError_t e = cudaMalloc((void **)&d_bad, 2 * sizeof(int));
+    if (e != cudaSuccess) { cudaFree(d_v); return fail(SW_ERR_NOMEM, "sw_selftest: cudaMalloc failed"); }
+    int bad[2] = { -1, -1 };
+    e = cudaMemcpy(d_v, v.data(), 4 * (size_t)n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(d_bad, 0, 2 * sizeof(int));
+    if (e == cudaSuccess) {
+        sw::k_selftest_compare<<<(n * n + 255) / 256, 256>>>(d_v, n, d_bad);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(bad, d_bad, sizeof(bad), cudaMemcpyDeviceToHost);
+    cudaFree(d_v);
+    cudaFree(d_bad);
+    if (e != cudaSuccess) return fail(SW_ERR_CUDA, "sw_selftest: %s", cudaGetErrorString(e));
+    if (bad[0] || bad[1])
+        return fail(SW_ERR_UNSUPPORTED, "sw_selftest: carry-flag compares disagree with >= (sub form %d, add form %d of %d pairs)", bad[0], bad[1], n * n);
+    return SW_OK;
+}
 
 const char *sw_last_error(void) { return g_err; }
 

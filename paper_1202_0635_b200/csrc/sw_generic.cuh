@@ -23,20 +23,24 @@ __device__ __forceinline__ void pdl_prologue()
     asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
+// Occupancy experiments only (SW_DUMMY_SMEM environment variable, read once by sw_create): unused dynamic shared memory
+// added to every PDL launch, to lower the number of resident CTAs per SM without touching the code.
+static unsigned g_pdl_dynamic_smem = 0;
+
 template <typename... Params, typename... Args>
-static inline void launch_pdl(void (*kernel)(Params...), unsigned grid, unsigned block, cudaStream_t stream, Args... args)
+static inline cudaError_t launch_pdl(void (*kernel)(Params...), unsigned grid, unsigned block, cudaStream_t stream, Args... args)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(block);
-    cfg.dynamicSmemBytes = 0;
+    cfg.dynamicSmemBytes = g_pdl_dynamic_smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
 }
 
 struct Model {
@@ -205,7 +209,7 @@ __device__ __forceinline__ uint32_t diff_mod_q(uint32_t s, uint32_t o, uint32_t 
 
 // sum the NB bins over the block's threads and add them to out[0..NB)
 template <int NB>
-__device__ __forceinline__ void hist_flush(unsigned int (*h)[HIST_THREADS], unsigned long long *__restrict__ out)
+__device__ __forceinline__ void hist_flush(unsigned int (*h)[HIST_THREADS], unsigned long long *out)
 {
     __syncthreads();
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -233,9 +237,10 @@ __device__ __forceinline__ uint32_t bytes_ne(uint32_t v, uint32_t d)
 // out[0..q) += bond_hist, out[16..16+q) += state_hist (unsigned long long, zeroed by the host).
 // L % 4 == 0: four sites per thread and iteration, counted in registers with byte-parallel compares (one counter
 // per value d < q; the loop over d is unrolled and cut off by the uniform test d < q), no shared-memory traffic.
+// `spins` is written by the previous kernel of the PDL chain (k_tile_flip): no const __restrict__, so that its loads stay
+// ordinary coherent loads ordered after griddepcontrol.wait (never ld.global.nc).
 template <int QB>   // QB = 2, 4, 8 or 16 >= q: bound of the unrolled loops over the values d
-__global__ void __launch_bounds__(HIST_THREADS) k_observables(Model md, const uint8_t *__restrict__ spins,
-                                                              unsigned long long *__restrict__ out)
+__global__ void __launch_bounds__(HIST_THREADS) k_observables(Model md, const uint8_t *spins, unsigned long long *out)
 {
     __shared__ unsigned int h[32][HIST_THREADS];
     const uint32_t tid = threadIdx.x;
@@ -290,8 +295,7 @@ __global__ void __launch_bounds__(HIST_THREADS) k_observables(Model md, const ui
 // Correlation histogram at distance r (eq.(5), (6); R15): out[d] += number of pairs (i, i + r e_x)
 // and (i, i + r e_y), periodic, with (S_i - S_{i+r}) mod q == d (unsigned long long, zeroed by the host).
 template <int QB>
-__global__ void __launch_bounds__(HIST_THREADS) k_correlation(Model md, const uint8_t *__restrict__ spins, uint32_t r,
-                                                              unsigned long long *__restrict__ out)
+__global__ void __launch_bounds__(HIST_THREADS) k_correlation(Model md, const uint8_t *spins, uint32_t r, unsigned long long *out)
 {
     __shared__ unsigned int h[16][HIST_THREADS];
     const uint32_t tid = threadIdx.x;

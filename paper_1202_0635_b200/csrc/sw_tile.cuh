@@ -144,15 +144,35 @@ __device__ __forceinline__ void ge_sub_shift_in(uint32_t &g, uint32_t w, uint32_
 {
     asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(g) : "r"(w), "r"(th));
 }
+// Device self-test of the two compare primitives above against the plain comparison (sw_selftest): the clock form
+// relies on the carry flag after sub.cc being "no borrow", which is what ptxas emits for sm_100a but not what the PTX
+// manual words, so a toolchain that changes it fails this test instead of silently flipping every clock bond.
+__global__ void k_selftest_compare(const uint32_t *vals, int n, int *bad)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n * n) return;
+    const uint32_t w = vals[i / n], th = vals[i % n];
+    const uint32_t ge = w >= th ? 1u : 0u;
+    uint32_t g1 = 2u, g2 = 2u;
+    ge_sub_shift_in(g2, w, th);
+    if (g2 != 4u + ge) atomicAdd(bad, 1);
+    if (th != 0u) {                       // the add form is only used with th > 0 (emask covers th == 0)
+        ge_shift_in(g1, w, 0u - th);
+        if (g1 != 4u + ge) atomicAdd(bad + 1, 1);
+    }
+}
+
 // K1.  grid = tiles, block = TILE_THREADS.  MODEL 0 = Potts, 1 = clock.
+// None of the kernels of the PDL chain qualifies a buffer that another kernel of the chain writes as const __restrict__:
+// such loads would compile to ld.global.nc, whose read-only contract does not hold while the producer grid may still be
+// draining, and which the "memory" clobber of griddepcontrol.wait does not order (tests/test_abi.py checks the SASS).
 #ifndef SW_LABEL_MINB
 #define SW_LABEL_MINB 5
 #endif
 template <int MODEL>
 __global__ void __launch_bounds__(TILE_THREADS, SW_LABEL_MINB)
-k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ spins, uint16_t *__restrict__ lab16,
-             unsigned long long *__restrict__ parent, uint32_t *__restrict__ hedge, uint32_t *__restrict__ vedge,
-             uint16_t *__restrict__ edges, uint32_t *__restrict__ ocount, int fuse, unsigned long long *stats)
+k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, uint16_t *lab16, unsigned long long *parent,
+             uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount, int fuse, unsigned long long *stats)
 {
     __shared__ uint32_t s_H[TH][NWORD];
     __shared__ uint32_t s_V[TH][NWORD];
@@ -653,7 +673,7 @@ __device__ __forceinline__ void gunion(unsigned long long *parent, uint32_t x, u
 }
 
 // read-only find (K3, label export): site index of the root of node x
-__device__ __forceinline__ uint32_t groot_site(const unsigned long long *__restrict__ parent, uint32_t x)
+__device__ __forceinline__ uint32_t groot_site(const unsigned long long *parent, uint32_t x)
 {
     unsigned long long p = __ldcg(parent + x);
     while ((uint32_t)p != x) { x = (uint32_t)p; p = __ldcg(parent + x); }
@@ -665,8 +685,8 @@ __device__ __forceinline__ uint32_t groot_site(const unsigned long long *__restr
 // from the compact edge arrays K1 wrote.
 constexpr int SEAM_THREADS = 256;
 __global__ void __launch_bounds__(SEAM_THREADS)
-k_seam_merge(Model md, const uint32_t *__restrict__ hedge, const uint32_t *__restrict__ vedge,
-             const uint16_t *__restrict__ edges, unsigned long long *parent, unsigned long long *stats)
+k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint16_t *edges, unsigned long long *parent,
+             unsigned long long *stats)
 {
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tiles_x = L / TW, tiles_y = L / TH;
@@ -700,9 +720,8 @@ k_seam_merge(Model md, const uint32_t *__restrict__ hedge, const uint32_t *__res
 // K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).  in = S^t, out = S^{t+1}.
 template <int MODEL>
 __global__ void __launch_bounds__(TILE_THREADS)
-k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ lab16,
-            const unsigned long long *__restrict__ parent, const uint32_t *__restrict__ ocount,
-            const uint8_t *__restrict__ in, uint8_t *__restrict__ out)
+k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *lab16, const unsigned long long *parent, const uint32_t *ocount,
+            const uint8_t *in, uint8_t *out)
 {
     constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
     __shared__ uint8_t s_dec[OCAP + NDEC];   // [pos] decision of the tile's open root pos; [DEC_BASE + d] = d
@@ -770,17 +789,19 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *__restrict__ la
 }
 
 // Debug export (sw_get_labels): canonical root of every site.
-__global__ void k_resolve_labels(Model md, const uint16_t *__restrict__ lab16, const unsigned long long *__restrict__ parent,
-                                 int32_t *__restrict__ out)
+// Sites first .. first + count - 1 -> out[0 .. count).
+__global__ void k_resolve_labels(Model md, const uint16_t *lab16, const unsigned long long *parent, uint32_t first, uint32_t count,
+                                 int32_t *out)
 {
     const uint32_t L = (uint32_t)md.L;
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= md.N) return;
+    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= count) return;
+    const uint32_t i = first + j;
     const uint32_t y = i / L, x = i - y * L;
     const uint32_t v = lab16[i];
     // written with fuse = 0: closed -> tile-local root sp; open -> LOPEN | pos
-    if (v & LOPEN) out[i] = (int32_t)groot_site(parent, ((y / TH) * (L / TW) + x / TW) * (uint32_t)OCAP + (v & (OCAP - 1u)));
-    else out[i] = (int32_t)root_site(v, x - x % TW, y - y % TH, L);
+    if (v & LOPEN) out[j] = (int32_t)groot_site(parent, ((y / TH) * (L / TW) + x / TW) * (uint32_t)OCAP + (v & (OCAP - 1u)));
+    else out[j] = (int32_t)root_site(v, x - x % TW, y - y % TH, L);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -807,16 +828,19 @@ static inline int tiled_init(TiledState &st, const Model &md, char *ws)
 constexpr int TILED_NUM_KERNELS = 3;
 static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k_seam_merge", "k_tile_flip" };
 
-static inline void tiled_launch_label(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
+static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
                                       unsigned long long *parent, int fuse, cudaStream_t stream, unsigned long long *stats)
 {
     const uint32_t tiles = ((uint32_t)md.L / TW) * ((uint32_t)md.L / TH);
+    if (g_pdl_dynamic_smem) {      // occupancy experiments only
+        cudaFuncSetAttribute(k_tile_label<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
+        cudaFuncSetAttribute(k_tile_label<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
+    }
     if (md.model == 0)
-        launch_pdl(k_tile_label<0>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
-                   st.ocount, fuse, stats);
-    else
-        launch_pdl(k_tile_label<1>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
-                   st.ocount, fuse, stats);
+        return launch_pdl(k_tile_label<0>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
+                          st.ocount, fuse, stats);
+    return launch_pdl(k_tile_label<1>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
+                      st.ocount, fuse, stats);
 }
 
 // One sweep: in = S^t (left untouched), out = S^{t+1}.  ev (optional): ev[0] is recorded before the first kernel,
@@ -829,14 +853,17 @@ static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &
     const uint32_t tiles = (L / TW) * (L / TH);
     const uint32_t ne = (L / TW) * L + (L / TH) * L;
     if (ev) cudaEventRecord(ev[0], stream);
-    tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats);
+    cudaError_t e = tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats);
+    if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[1], stream);
-    launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent, stats);
+    e = launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent, stats);
+    if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[2], stream);
     if (md.model == 0)
-        launch_pdl(k_tile_flip<0>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out);
+        e = launch_pdl(k_tile_flip<0>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out);
     else
-        launch_pdl(k_tile_flip<1>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out);
+        e = launch_pdl(k_tile_flip<1>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out);
+    if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[3], stream);
     *launches += 3;
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
@@ -845,14 +872,23 @@ static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &
 // Debug export (sw_get_labels): label the configuration `in` with the bonds of sweep t again, this time keeping the
 // tile-local root of every site (no fused decisions), merge, and resolve every site to its canonical root.
 static inline int tiled_relabel(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
-                                unsigned long long *parent, int32_t *out, cudaStream_t stream, uint64_t *launches)
+                                unsigned long long *parent, cudaStream_t stream, uint64_t *launches)
 {
     const uint32_t L = (uint32_t)md.L;
     const uint32_t ne = (L / TW) * L + (L / TH) * L;
-    tiled_launch_label(st, md, key, t, in, parent, 0, stream, nullptr);
-    launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent, (unsigned long long *)nullptr);
-    k_resolve_labels<<<(md.N + 255) / 256, 256, 0, stream>>>(md, st.lab16, parent, out);
-    *launches += 3;
+    if (tiled_launch_label(st, md, key, t, in, parent, 0, stream, nullptr) != cudaSuccess) return -1;
+    if (launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent,
+                   (unsigned long long *)nullptr) != cudaSuccess) return -1;
+    *launches += 2;
+    return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
+}
+
+// ... and resolve sites first .. first + count - 1 to their canonical roots, out[0 .. count).
+static inline int tiled_resolve_chunk(TiledState &st, const Model &md, const unsigned long long *parent, uint32_t first, uint32_t count,
+                                      int32_t *out, cudaStream_t stream, uint64_t *launches)
+{
+    k_resolve_labels<<<(count + 255) / 256, 256, 0, stream>>>(md, st.lab16, parent, first, count, out);
+    *launches += 1;
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
 }
 

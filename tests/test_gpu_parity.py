@@ -143,11 +143,14 @@ def test_composition_resume_and_record(sw, oracle, algo, L):
         _assert_same(sh, osh, "recorded state_hist")
         _assert_same(a.get_spins(), s_or, "spins after sweep_record")
         assert a.sweep_index == 18
-        # derived doubles (R11) from both sides' integers: within 1e-12 relative (identical in fact)
+        # derived doubles (R11): the library's sw_derive_* on the GPU's integers against the ORACLE's own functions on
+        # the oracle's integers, 1e-12 relative (north_star)
         for k in range(6):
-            e_gpu, e_or = sw.potts_energy(L, bh[k]), sw.potts_energy(L, obh[k])
-            m_gpu, m_or = sw.potts_m2(q, sh[k]), sw.potts_m2(q, osh[k])
+            e_gpu, e_or = sw.potts_energy(L, bh[k]), oracle.potts_energy(L, obh[k])
+            m_gpu, m_or = sw.potts_m2(q, sh[k]), oracle.potts_m2(q, osh[k])
             assert abs(e_gpu - e_or) <= 1e-12 * abs(e_or) and abs(m_gpu - m_or) <= 1e-12 * max(1.0, abs(m_or))
+        u_gpu, u_or = sw.moment_ratio(q, sh), oracle.moment_ratio(q, osh)
+        assert abs(u_gpu - u_or) <= 1e-12 * abs(u_or) and u_or >= 1.0
 
 
 def test_set_spins_rejects_bad_values_and_errors(sw):
@@ -181,9 +184,9 @@ def test_clock_record_and_observables(sw, oracle):
         _assert_same(sh, osh, "clock state_hist")
         _assert_same(lat.get_spins(), s_or, "clock spins")
         for k in range(5):
-            a, b = sw.clock_energy(q, bh[k]), sw.clock_energy(q, obh[k])
+            a, b = sw.clock_energy(q, bh[k]), oracle.clock_energy(q, obh[k])
             assert abs(a - b) <= 1e-12 * abs(b)
-            assert abs(sw.clock_magnetisation(q, sh[k]) - sw.clock_magnetisation(q, osh[k])) <= 1e-12 * L * L
+            assert abs(sw.clock_m(q, sh[k]) - oracle.clock_m(q, osh[k])) <= 1e-12 * L * L
 
 
 # ------------------------------------------------------------------------------------------------
@@ -205,35 +208,48 @@ def test_config1_L64_every_one_of_1000_sweeps(sw, oracle):
         assert np.array_equal(bh, obh) and np.array_equal(sh, osh)
 
 
-def _snapshot_check(sw, oracle, w, early, late_at, late):
-    """Sweeps 0..early-1 compared one by one; then the GPU runs alone to sweep `late_at`, and `late` further sweeps
-    are compared starting from GPU snapshots handed to the oracle (spins, t).  Oracle sweeps run in parallel threads:
-    each one starts from a GPU snapshot, so they are independent checks."""
+def _largest_cluster_fraction(labels):
+    lab = np.asarray(labels).ravel()
+    return float(np.bincount(lab).max()) / lab.size
+
+
+def _snapshot_check(sw, oracle, w, early, lates, regime=None):
+    """Sweeps 0..early-1 compared one by one; then, for every (t_at, n) of `lates`, the GPU runs alone to sweep t_at
+    and n further sweeps are compared starting from GPU snapshots handed to the oracle (spins, t) -- SURVEY 8(c) row
+    "GPU vs oracle".  Oracle sweeps run in parallel threads: each one starts from a GPU snapshot, so they are independent
+    checks.  `regime` = (t, lo, hi): the largest-cluster fraction of the oracle's labels of sweep t (one of the compared
+    sweeps) must lie in [lo, hi], so that a reader sees which cluster structure the snapshot exercised."""
     jobs = []  # (t, spins_before, spins_after_gpu, obs_before_gpu)
     with sw.Lattice(w.L, w.q, w.model, w.T, w.seed) as lat:
         assert lat.algorithm == TILED
         _assert_same(lat.get_thresholds(), oracle.thresholds(w.q, w.model, w.T), "thresholds")
         s_before = lat.get_spins()
         _assert_same(s_before, oracle.init_spins(w.L, w.q, w.seed), "initial spins")
-        for t in range(early):
-            obs = lat.observables()
-            lat.sweep(1)
-            s_after = lat.get_spins()
-            jobs.append((t, s_before, s_after, obs))
-            s_before = s_after
-        if late:
-            lat.sweep(late_at - early)
-            s_before = lat.get_spins()
-            for t in range(late_at, late_at + late):
+        t_now = 0
+        for t_at, n in [(0, early)] + list(lates):
+            if n == 0:
+                continue
+            if t_at > t_now:
+                lat.sweep(t_at - t_now)
+                s_before = lat.get_spins()
+            assert lat.sweep_index == t_at
+            for t in range(t_at, t_at + n):
                 obs = lat.observables()
                 lat.sweep(1)
                 s_after = lat.get_spins()
                 jobs.append((t, s_before, s_after, obs))
                 s_before = s_after
+            t_now = t_at + n
+
+    fractions = {}
 
     def check(job):
         t, sb, sa, (bh, sh) = job
-        want = oracle.sweep(w.L, w.q, w.model, w.T, w.seed, t, sb)
+        if regime is not None and t == regime[0]:
+            want, lab = oracle.sweep(w.L, w.q, w.model, w.T, w.seed, t, sb, want_labels=True)
+            fractions[t] = _largest_cluster_fraction(lab)
+        else:
+            want = oracle.sweep(w.L, w.q, w.model, w.T, w.seed, t, sb)
         obh, osh = oracle.observables(w.L, w.q, sb)
         return t, np.array_equal(want, sa), np.array_equal(bh, obh) and np.array_equal(sh, osh)
 
@@ -241,30 +257,62 @@ def _snapshot_check(sw, oracle, w, early, late_at, late):
         for t, ok_s, ok_o in ex.map(check, jobs):
             assert ok_s, f"{w.name}: spins after sweep {t} differ from the oracle"
             assert ok_o, f"{w.name}: observables before sweep {t} differ from the oracle"
+    if regime is not None:
+        f = fractions[regime[0]]
+        print(f"{w.name}: largest cluster of sweep {regime[0]} holds {f:.4f} of the sites")
+        assert regime[1] <= f <= regime[2], f"{w.name}: largest-cluster fraction {f} outside [{regime[1]}, {regime[2]}] at sweep {regime[0]}"
 
 
 def test_config2_L4096_potts2(sw, oracle):
+    """sweeps 0..32 one by one, then snapshots at t = 1000, 6000, 10990 (the last sweeps of the config's
+    1000 + 10000), a few sweeps each.  At Tc the largest cluster holds a sizeable fraction (L^(-1/8) scaling)."""
     from paper_1202_0635_b200.workloads import CONFIGS
-    _snapshot_check(sw, oracle, CONFIGS["c2_potts2_L4096"], early=3, late_at=300, late=3)
+    _snapshot_check(sw, oracle, CONFIGS["c2_potts2_L4096"], early=33, lates=[(1000, 3), (6000, 3), (10990, 3)], regime=(6001, 0.05, 0.8))
 
 
 def test_config3_L4096_clock6(sw, oracle):
     from paper_1202_0635_b200.workloads import CONFIGS
-    _snapshot_check(sw, oracle, CONFIGS["c3_clock6_L4096"], early=2, late_at=200, late=2)
+    _snapshot_check(sw, oracle, CONFIGS["c3_clock6_L4096"], early=12, lates=[(1000, 2), (9990, 2)], regime=(1001, 0.0, 0.9))
 
 
 def test_config4_L8192_potts3_and_4(sw, oracle):
     from paper_1202_0635_b200.workloads import CONFIGS
-    _snapshot_check(sw, oracle, CONFIGS["c4_potts3_L8192"], early=1, late_at=100, late=1)
-    _snapshot_check(sw, oracle, CONFIGS["c4_potts4_L8192"], early=1, late_at=100, late=1)
+    _snapshot_check(sw, oracle, CONFIGS["c4_potts3_L8192"], early=3, lates=[(1000, 2)], regime=(1001, 0.0, 0.8))
+    _snapshot_check(sw, oracle, CONFIGS["c4_potts4_L8192"], early=3, lates=[(1000, 2)], regime=(1001, 0.0, 0.8))
 
 
 def test_config5_L16384_three_temperatures(sw, oracle):
-    """Late snapshots matter: the spanning cluster at 0.8 Tc does not exist at t = 0."""
+    """Late snapshots matter: the spanning cluster at 0.8 Tc does not exist at t = 0.  At t = 300 it does (SURVEY 8(d):
+    "one cluster holds 95 % of sites"); at 1.2 Tc the largest cluster is tiny."""
     from paper_1202_0635_b200.workloads import CONFIGS
-    _snapshot_check(sw, oracle, CONFIGS["c5_potts2_L16384_0.8Tc"], early=1, late_at=60, late=1)
-    _snapshot_check(sw, oracle, CONFIGS["c5_potts2_L16384_Tc"], early=0, late_at=60, late=1)
-    _snapshot_check(sw, oracle, CONFIGS["c5_potts2_L16384_1.2Tc"], early=0, late_at=60, late=1)
+    _snapshot_check(sw, oracle, CONFIGS["c5_potts2_L16384_0.8Tc"], early=1, lates=[(300, 2)], regime=(301, 0.85, 1.0))
+    _snapshot_check(sw, oracle, CONFIGS["c5_potts2_L16384_Tc"], early=1, lates=[(300, 1)], regime=(300, 0.01, 0.8))
+    _snapshot_check(sw, oracle, CONFIGS["c5_potts2_L16384_1.2Tc"], early=0, lates=[(300, 1)], regime=(300, 0.0, 0.01))
+
+
+@pytest.mark.parametrize("L", [4096, 16384])
+def test_full_size_structured_start_one_giant_root(sw, oracle, L):
+    """A uniform lattice handed in at full size, cold (T = 0.02: every bond active, ONE cluster) and at 0.8 Tc (p = 0.67,
+    a spanning cluster with holes): every tile's open roots funnel into one global root -- the worst case of the
+    cross-tile union-find (2048 tiles at L = 4096, 32768 at L = 16384).  Spins AND canonical labels of two sweeps."""
+    from paper_1202_0635_b200.workloads import uniform_spins
+    q, seed, t0 = 2, 0x5EED0005, 5
+    for T, lo in ((0.02, 0.999), (0.8 * tc(2), 0.85)):
+        with sw.Lattice(L, q, POTTS, T, seed) as lat:
+            assert lat.algorithm == TILED
+            s = uniform_spins(L, 1)
+            lat.set_spins(s, t0)
+            for t in range(t0, t0 + 2):
+                lat.sweep(1)
+                s_gpu, lab_gpu = lat.get_spins(), lat.get_labels()
+                s, olab = oracle.sweep(L, q, POTTS, T, seed, t, s, want_labels=True)
+                _assert_same(lab_gpu, olab, f"L={L} T={T}: labels of sweep {t}")
+                _assert_same(s_gpu, s, f"L={L} T={T}: spins after sweep {t}")
+                if t == t0:
+                    f = _largest_cluster_fraction(olab)
+                    print(f"L={L} T={T:.4f}: largest cluster holds {f:.5f} of the sites")
+                    assert f >= lo
+                del lab_gpu, olab
 
 
 # ------------------------------------------------------------------------------------------------
@@ -289,6 +337,7 @@ def test_record_corr_rows_and_derived_doubles(sw, oracle):
     with sw.Lattice(L, q, CLOCK, T, seed) as lat:
         bh, sh, c1, c2 = lat.sweep_record_corr(n, L // 4, L // 2)
     s = oracle.init_spins(L, q, seed)
+    oq, oh = [], []
     for k in range(n):
         obh, osh = oracle.observables(L, q, s)
         _assert_same(bh[k], obh, f"bond row {k}")
@@ -296,9 +345,12 @@ def test_record_corr_rows_and_derived_doubles(sw, oracle):
         o1, o2 = oracle.correlation(L, q, s, L // 4), oracle.correlation(L, q, s, L // 2)
         _assert_same(c1[k], o1, f"corr(L/4) row {k}")
         _assert_same(c2[k], o2, f"corr(L/2) row {k}")
-        g1, g2 = sw.correlation_g(q, c1[k]), sw.correlation_g(q, o1)
-        assert g1 == g2 and abs(g1) <= 1.0
+        oq.append(o1); oh.append(o2)
+        g_gpu, g_or = sw.g(q, c1[k]), oracle.g(q, o1)             # eq.(5): library vs oracle, 1e-12 relative
+        assert abs(g_gpu - g_or) <= 1e-12 * max(abs(g_or), 1e-300) and abs(g_gpu) <= 1.0
         s = oracle.sweep(L, q, CLOCK, T, seed, k, s)
+    r_gpu, r_or = sw.ratio_R(q, c2, c1), oracle.ratio_R(q, np.array(oh), np.array(oq))   # eq.(6)
+    assert abs(r_gpu - r_or) <= 1e-12 * abs(r_or)
 
 
 def test_correlation_full_size_sampled(sw, oracle):
