@@ -100,6 +100,7 @@ struct sw_ctx {
     int last_algo = 0;
     uint64_t launches = 0, stat_sweeps = 0;
     sw::TiledState tiled{};
+    unsigned long long *rec_host = nullptr;   // pinned copy of the record ring (sw_sweep_record)
 };
 
 namespace {
@@ -168,13 +169,17 @@ int generic_sweep(sw_ctx *c, uint32_t t, cudaEvent_t *ev)
     return SW_OK;
 }
 
-int one_sweep(sw_ctx *c, cudaEvent_t *ev = nullptr)
+// obs_row (optional): zeroed row of the record ring that receives the observables of S^t if the back-end fuses S5 into
+// its first kernel (fuses_observables); otherwise the caller has launched k_observables on it already.
+bool fuses_observables(const sw_ctx *c) { return c->algo == SW_ALGO_TILED && sw::tiled_fuses_observables(c->md); }
+
+int one_sweep(sw_ctx *c, cudaEvent_t *ev = nullptr, unsigned long long *obs_row = nullptr)
 {
     const uint32_t t = (uint32_t)c->t;
     int rc;
     if (c->algo == SW_ALGO_TILED) {
         rc = sw::tiled_sweep(c->tiled, c->md, c->key, t, c->spins, c->spins_alt, (unsigned long long *)c->labels, c->stream,
-                             c->stats_on ? c->stats : nullptr, &c->launches, ev);
+                             c->stats_on ? c->stats : nullptr, &c->launches, ev, obs_row);
         if (rc != 0) return fail(SW_ERR_CUDA, "tiled sweep launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         std::swap(c->spins, c->spins_alt);   // spins_alt now holds S^t, the input of this sweep
     } else {
@@ -281,6 +286,12 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
     c->tiled_ws = c->ws + c->cv.tiled;
     c->key = sw::make_philox_key(seed);
     build_thresholds(c);
+    if (cudaMallocHost((void **)&c->rec_host, (size_t)REC_ROWS * OBS_WORDS * 8) != cudaSuccess) {
+        fail(SW_ERR_NOMEM, "sw_create: cudaMallocHost failed: %s", cudaGetErrorString(cudaGetLastError()));
+        c->rec_host = nullptr;
+        sw_destroy(c);
+        return nullptr;
+    }
     c->md.L = L; c->md.q = q; c->md.model = model; c->md.N = (uint32_t)c->N;
     c->md.thr_potts = (model == SW_POTTS) ? c->thr_host[0] : 0u;
     c->md.table = c->table;
@@ -331,6 +342,7 @@ void sw_destroy(sw_ctx *c)
     if (!c) return;
     DeviceGuard guard(c);
     if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
+    if (c->rec_host) cudaFreeHost(c->rec_host);
     if (c->own_ws && c->ws) cudaFree(c->ws);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
     delete c;
@@ -369,25 +381,26 @@ namespace {
 // r1 < 0: no correlation histograms.
 int record_impl(sw_ctx *c, int n, int r1, int r2, int64_t *bond_out, int64_t *state_out, int64_t *c1_out, int64_t *c2_out)
 {
-    std::vector<unsigned long long> host((size_t)REC_ROWS * OBS_WORDS);
+    unsigned long long *host = c->rec_host;   // pinned staging buffer of the ring (allocated with the context)
+    const bool fused = fuses_observables(c);
     int done = 0;
     while (done < n) {
         const int chunk = std::min(REC_ROWS, n - done);
         CU_TRY(cudaMemsetAsync(c->ring, 0, (size_t)chunk * OBS_WORDS * 8, c->stream));   // all rows of the chunk at once
         for (int k = 0; k < chunk; ++k) {
             unsigned long long *row = c->ring + (size_t)k * OBS_WORDS;
-            int rc = launch_observables(c, row, false);
+            int rc = fused ? SW_OK : launch_observables(c, row, false);
             if (rc != SW_OK) return rc;
             if (r1 >= 0) {
                 rc = launch_correlation(c, r1, row + 32);
                 if (rc == SW_OK) rc = launch_correlation(c, r2, row + 48);
                 if (rc != SW_OK) return rc;
             }
-            rc = one_sweep(c);
+            rc = one_sweep(c, nullptr, fused ? row : nullptr);
             if (rc != SW_OK) return rc;
         }
         CU_TRY(cudaGetLastError());
-        CU_TRY(cudaMemcpyAsync(host.data(), c->ring, (size_t)chunk * OBS_WORDS * 8, cudaMemcpyDeviceToHost, c->stream));
+        CU_TRY(cudaMemcpyAsync(host, c->ring, (size_t)chunk * OBS_WORDS * 8, cudaMemcpyDeviceToHost, c->stream));
         CU_TRY(cudaStreamSynchronize(c->stream));
         for (int k = 0; k < chunk; ++k)
             for (int j = 0; j < c->q; ++j) {

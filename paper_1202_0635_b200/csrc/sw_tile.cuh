@@ -169,18 +169,28 @@ __global__ void k_selftest_compare(const uint32_t *vals, int n, int *bad)
 #ifndef SW_LABEL_MINB
 #define SW_LABEL_MINB 5
 #endif
-template <int MODEL>
+template <int MODEL, bool OBS>
 __global__ void __launch_bounds__(TILE_THREADS, SW_LABEL_MINB)
 k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, uint16_t *lab16, unsigned long long *parent,
-             uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount, int fuse, unsigned long long *stats)
+             uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount, int fuse, unsigned long long *stats,
+             unsigned long long *obs)
 {
+    // OBS (q = 2 Potts only, "+ measurement" of PAPER.md:75): S5 fused into phase A.  With two states the
+    // XOR of a spin word with its +x / +y neighbour word has byte 1 exactly on the unequal bonds, so three POPC per four
+    // sites (on the otherwise idle XU pipe) give bond_hist[1] and state_hist[1] of S^t; the other two bins follow from
+    // the tile's site count.  obs[0..1] += bond_hist, obs[16..17] += state_hist (one row of the record ring).
+    __shared__ uint32_t s_obs[2];
     __shared__ uint32_t s_H[TH][NWORD];
     __shared__ uint32_t s_V[TH][NWORD];
     __shared__ uint32_t s_lab[LAB_WORDS];
     __shared__ uint32_t s_nopen;
     __shared__ uint32_t s_edge[TILE_THREADS / 32][EDGE_CAP + 1];   // + dump slot
     __shared__ uint32_t s_enext[TILE_THREADS / 32];                 // next edge to hand out, per warp
-    __shared__ uint32_t s_table[MODEL == 1 ? (2 * 16) * (2 * 16) : 1];
+    // clock threshold table (phase A only): it lives in the edge lists, which nobody touches before phase B -- a table of
+    // its own (4 KB) would cost the fifth resident CTA per SM
+    constexpr bool TABLE_ALIAS = (TILE_THREADS / 32) * (EDGE_CAP + 1) >= (2 * 16) * (2 * 16);
+    __shared__ uint32_t s_table_own[(MODEL == 1 && !TABLE_ALIAS) ? (2 * 16) * (2 * 16) : 1];
+    uint32_t *const s_table = TABLE_ALIAS ? &s_edge[0][0] : s_table_own;
 
     pdl_prologue();
     const uint32_t L = (uint32_t)md.L;
@@ -200,6 +210,10 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, uint16_t
     static_assert(2 * (EDGE_CAP + 1) >= RCAP, "closed-root list must fit the warp's edge list");
     uint32_t m = 0u;
     if (tid == 32u) s_nopen = 0u;
+    if (OBS && tid < 2u) s_obs[tid] = 0u;
+    if (OBS) __syncthreads();
+    uint32_t o_neq = 0u, o_one = 0u;
+    (void)o_neq; (void)o_one; (void)s_obs;
     if (MODEL == 1) {
         for (uint32_t k = tid; k < q2 * q2; k += TILE_THREADS) s_table[k] = md.table[k];
         m = axis_of_sweep(key, t, (uint32_t)md.q);
@@ -242,6 +256,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, uint16_t
                 // [w >= th] is the carry of w + (2^32 - th); add-with-carry shifts it into a nibble (two ALU instructions
                 // per bond instead of compare + select + or); equal spins come from a zero-byte test on the XOR.
                 const uint32_t dx = cur ^ right, dy = cur ^ nxt;   // byte k zero <=> equal spins (bytes < 16)
+                if (OBS) { o_neq += (uint32_t)__popc(dx) + (uint32_t)__popc(dy); o_one += (uint32_t)__popc(cur); }
                 const uint32_t zx = ~(dx + 0x7F7F7F7Fu) & emask, zy = ~(dy + 0x7F7F7F7Fu) & emask;
                 const uint32_t eqh = (zx * 0x00204081u) >> 28, eqv = (zy * 0x00204081u) >> 28;   // bits 7,15,23,31 -> 0..3
                 uint32_t gh = 0u, gv = 0u;
@@ -272,7 +287,17 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, uint16_t
             }
         }
     }
+    if (OBS) {
+        o_neq = __reduce_add_sync(0xFFFFFFFFu, o_neq);
+        o_one = __reduce_add_sync(0xFFFFFFFFu, o_one);
+        if (lane == 0u) { atomicAdd(&s_obs[0], o_neq); atomicAdd(&s_obs[1], o_one); }
+    }
     __syncthreads();
+    if (OBS && tid < 4u) {
+        const uint32_t neq = s_obs[0], one = s_obs[1];
+        const uint32_t v = tid == 0u ? 2u * TILE_SITES - neq : tid == 1u ? neq : tid == 2u ? TILE_SITES - one : one;
+        atomicAdd(obs + (tid < 2u ? tid : 14u + tid), (unsigned long long)v);
+    }
 
     SW_PHASE(0)
     // bonds that leave the tile: exported for K2, never used by the tile-local graph below
@@ -680,6 +705,18 @@ __device__ __forceinline__ uint32_t groot_site(const unsigned long long *parent,
     return (uint32_t)(p >> 32);
 }
 
+// find with write-back (K3): the node itself is re-pointed to the root, so chases of other tiles that pass through it
+// end one hop later.  A racing reader sees the old parent or the root: both are ancestors.
+__device__ __forceinline__ uint32_t groot_site_compress(unsigned long long *parent, uint32_t x)
+{
+    const uint32_t x0 = x;
+    unsigned long long p = __ldcg(parent + x);
+    uint32_t hops = 0u;
+    while ((uint32_t)p != x) { x = (uint32_t)p; p = __ldcg(parent + x); ++hops; }
+    if (hops > 1u) __stcg(parent + x0, p);
+    return (uint32_t)(p >> 32);
+}
+
 // K2.  One thread per tile-edge bond position: first the (L/128)*L right-edge bonds, then the (L/TH)*L bottom-edge
 // bonds.  The two ends of an active tile-crossing bond lie in open clusters; their lab16 values (LOPEN | pos) come
 // from the compact edge arrays K1 wrote.
@@ -712,7 +749,13 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
         ib = 2 * TH + x % TW;                 // top row of tb
     }
     const uint32_t a = edges[(size_t)ta * ECNT + ia], b = edges[(size_t)tb * ECNT + ib];
+    const uint32_t act = __ballot_sync(0xFFFFFFFFu, bit != 0u);   // ne is a multiple of 32: whole warps get here
     if (!bit) return;
+    // The 32 positions of a warp lie on one seam of one pair of tiles (32 | TH, 32 | TW), and neighbouring bonds mostly
+    // join the same two clusters: one lane per distinct (a, b) pair does the union (SURVEY 7 hard part 3).
+    const uint32_t pair = (a << 16) | (b & 0xFFFFu);
+    const uint32_t same = __match_any_sync(act, pair);
+    if ((uint32_t)__ffs((int)same) - 1u != (threadIdx.x & 31u)) return;
     if (stats) atomicAdd(stats + 1, 1ull);
     gunion(parent, ta * OCAP + (a & (OCAP - 1u)), tb * OCAP + (b & (OCAP - 1u)));
 }
@@ -720,7 +763,7 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
 // K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).  in = S^t, out = S^{t+1}.
 template <int MODEL>
 __global__ void __launch_bounds__(TILE_THREADS)
-k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *lab16, const unsigned long long *parent, const uint32_t *ocount,
+k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *lab16, unsigned long long *parent, const uint32_t *ocount,
             const uint8_t *in, uint8_t *out)
 {
     constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
@@ -737,7 +780,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *lab16, const un
     // of its cluster in the global union-find
     const uint32_t no = ocount[blockIdx.x];
     uint32_t r = 0u;
-    if (tid < no) r = groot_site(parent, blockIdx.x * (uint32_t)OCAP + tid);
+    if (tid < no) r = groot_site_compress(parent, blockIdx.x * (uint32_t)OCAP + tid);
     uint4 lab[PASSES];
 #pragma unroll
     for (int c = 0; c < PASSES; ++c) {
@@ -746,7 +789,7 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *lab16, const un
     }
     if (tid < (uint32_t)NDEC) s_dec[DEC_BASE + tid] = (uint8_t)tid;
     for (uint32_t i = tid; i < no; i += TILE_THREADS) {
-        if (i >= TILE_THREADS) r = groot_site(parent, blockIdx.x * (uint32_t)OCAP + i);
+        if (i >= TILE_THREADS) r = groot_site_compress(parent, blockIdx.x * (uint32_t)OCAP + i);
         uint32_t w[4];
         philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
         const uint32_t ww = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
@@ -829,31 +872,38 @@ constexpr int TILED_NUM_KERNELS = 3;
 static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k_seam_merge", "k_tile_flip" };
 
 static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
-                                      unsigned long long *parent, int fuse, cudaStream_t stream, unsigned long long *stats)
+                                      unsigned long long *parent, int fuse, cudaStream_t stream, unsigned long long *stats,
+                                      unsigned long long *obs = nullptr)
 {
     const uint32_t tiles = ((uint32_t)md.L / TW) * ((uint32_t)md.L / TH);
     if (g_pdl_dynamic_smem) {      // occupancy experiments only
-        cudaFuncSetAttribute(k_tile_label<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
-        cudaFuncSetAttribute(k_tile_label<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
+        cudaFuncSetAttribute(k_tile_label<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
+        cudaFuncSetAttribute(k_tile_label<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
     }
+    if (md.model == 0 && md.q == 2 && obs)
+        return launch_pdl(k_tile_label<0, true>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge,
+                          st.edges, st.ocount, fuse, stats, obs);
     if (md.model == 0)
-        return launch_pdl(k_tile_label<0>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
-                          st.ocount, fuse, stats);
-    return launch_pdl(k_tile_label<1>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
-                      st.ocount, fuse, stats);
+        return launch_pdl(k_tile_label<0, false>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge,
+                          st.edges, st.ocount, fuse, stats, (unsigned long long *)nullptr);
+    return launch_pdl(k_tile_label<1, false>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
+                      st.ocount, fuse, stats, (unsigned long long *)nullptr);
 }
 
 // One sweep: in = S^t (left untouched), out = S^{t+1}.  ev (optional): ev[0] is recorded before the first kernel,
 // ev[k+1] after kernel k.
+// obs (optional, zeroed row of the record ring): K1 adds the observables of S^t to it when it can (tiled_fuses_observables).
+static inline bool tiled_fuses_observables(const Model &md) { return md.model == 0 && md.q == 2; }
+
 static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
                               uint8_t *out, unsigned long long *parent, cudaStream_t stream, unsigned long long *stats,
-                              uint64_t *launches, cudaEvent_t *ev)
+                              uint64_t *launches, cudaEvent_t *ev, unsigned long long *obs = nullptr)
 {
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tiles = (L / TW) * (L / TH);
     const uint32_t ne = (L / TW) * L + (L / TH) * L;
     if (ev) cudaEventRecord(ev[0], stream);
-    cudaError_t e = tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats);
+    cudaError_t e = tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats, obs);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[1], stream);
     e = launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent, stats);
