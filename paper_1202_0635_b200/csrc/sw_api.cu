@@ -307,7 +307,7 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
         ok = cudaGetLastError() == cudaSuccess;
     }
     c->algo = sw::tiled_supported(L) ? SW_ALGO_TILED : SW_ALGO_GENERIC;
-    if (ok && sw::tiled_supported(L)) ok = sw::tiled_init(c->tiled, c->md, c->tiled_ws) == 0;
+    if (ok && sw::tiled_supported(L)) ok = sw::tiled_init(c->tiled, c->md, c->tiled_ws, c->spins, c->spins_alt) == 0;
     ok = ok && cudaStreamSynchronize(c->stream) == cudaSuccess;
     if (!ok) {
         fail(SW_ERR_CUDA, "sw_create: device initialisation failed: %s", cudaGetErrorString(cudaGetLastError()));

@@ -25,6 +25,7 @@
 // of the global indices), so spins, labels and observables equal the oracle's bit for bit.
 // HBM traffic per site and sweep: K1 1 B (spins) + 2 B (labels); K3 2 B (labels) [+ 1 B spins, clock] + 1 B.
 #pragma once
+#include <cuda.h>            // CUtensorMap (types only: the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -32,6 +33,36 @@
 #include "sw_philox.cuh"
 
 namespace sw {
+
+// ---- TMA (cp.async.bulk.tensor) + mbarrier, raw PTX ---------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "SW_MBAR_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra SW_MBAR_DONE;\n\t"
+        "bra SW_MBAR_WAIT;\n\t"
+        "SW_MBAR_DONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// one box of a 2D tensor map -> shared memory, completion counted in bytes on the mbarrier
+__device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *map, uint32_t x, uint32_t y, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(reinterpret_cast<uint64_t>(map)), "r"(x), "r"(y), "r"(smem_u32(bar))
+                 : "memory");
+}
 
 constexpr int TW = 128;                 // sites per tile row = 4 words of 32
 constexpr int TH = 64;                  // rows per tile
@@ -64,6 +95,9 @@ struct TiledState {
     uint16_t *edges = nullptr;   // [tiles][ECNT]  lab16 values of the tile's boundary sites: left col, right col, top row, bottom row
     uint32_t *ocount = nullptr;  // [tiles]        how many
     int L = 0;
+    // TMA: one tensor map per spin buffer of the ping-pong ([L][L] uint8, box = one 128 x 64 tile)
+    const uint8_t *map_base[2] = { nullptr, nullptr };
+    CUtensorMap map[2];
 };
 
 static inline bool tiled_supported(int L) { return L >= TW && L % TW == 0 && L % TH == 0; }
@@ -169,11 +203,15 @@ __global__ void k_selftest_compare(const uint32_t *vals, int n, int *bad)
 #ifndef SW_LABEL_MINB
 #define SW_LABEL_MINB 5
 #endif
+// The 128 x 64 spin bytes of the tile are staged in shared memory by TMA: one cp.async.bulk.tensor box issued by one
+// thread, completion on an mbarrier; it lands in the storage of the edge lists, which phase B only starts to use after
+// phase A has consumed the spins.  The periodic halo (row below, column to the right: tensor maps do not wrap) comes
+// through plain loads issued while the box is in flight.
 template <int MODEL, bool OBS>
 __global__ void __launch_bounds__(TILE_THREADS, SW_LABEL_MINB)
-k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, uint16_t *lab16, unsigned long long *parent,
-             uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount, int fuse, unsigned long long *stats,
-             unsigned long long *obs)
+k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, const __grid_constant__ CUtensorMap spin_map,
+             uint16_t *lab16, unsigned long long *parent, uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount,
+             int fuse, unsigned long long *stats, unsigned long long *obs)
 {
     // OBS (q = 2 Potts only, "+ measurement" of PAPER.md:75): S5 fused into phase A.  With two states the
     // XOR of a spin word with its +x / +y neighbour word has byte 1 exactly on the unequal bonds, so three POPC per four
@@ -184,14 +222,19 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, uint16_t
     __shared__ uint32_t s_V[TH][NWORD];
     __shared__ uint32_t s_lab[LAB_WORDS];
     __shared__ uint32_t s_nopen;
-    __shared__ uint32_t s_edge[TILE_THREADS / 32][EDGE_CAP + 1];   // + dump slot
+    // s_ew: phase A reads the TMA-staged spins of the tile from it (TILE_SITES bytes), phase B keeps the per-warp edge
+    // lists in it ([warp][EDGE_CAP + 1], + dump slot): the two uses never overlap in time
+    constexpr int EDGE_WORDS = (TILE_THREADS / 32) * (EDGE_CAP + 1);
+    constexpr int EW_WORDS = EDGE_WORDS > TILE_SITES / 4 ? EDGE_WORDS : TILE_SITES / 4;
+    __shared__ __align__(128) uint32_t s_ew[EW_WORDS];
+    uint32_t(*const s_edge)[EDGE_CAP + 1] = reinterpret_cast<uint32_t(*)[EDGE_CAP + 1]>(s_ew);
     __shared__ uint32_t s_enext[TILE_THREADS / 32];                 // next edge to hand out, per warp
-    // clock threshold table (phase A only): it lives in the edge lists, which nobody touches before phase B -- a table of
-    // its own (4 KB) would cost the fifth resident CTA per SM
-    constexpr bool TABLE_ALIAS = (TILE_THREADS / 32) * (EDGE_CAP + 1) >= (2 * 16) * (2 * 16);
-    __shared__ uint32_t s_table_own[(MODEL == 1 && !TABLE_ALIAS) ? (2 * 16) * (2 * 16) : 1];
-    uint32_t *const s_table = TABLE_ALIAS ? &s_edge[0][0] : s_table_own;
+    __shared__ __align__(8) unsigned long long s_bar;               // mbarrier of the staged box
+    // clock threshold table (phase A only): it lives in the label array, which nobody touches before phase B -- a table
+    // of its own (4 KB) would cost the fifth resident CTA per SM
+    uint32_t *const s_table = s_lab;
 
+    if (threadIdx.x == 0u) mbar_init(&s_bar, 1u);
     pdl_prologue();
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -211,13 +254,15 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, uint16_t
     uint32_t m = 0u;
     if (tid == 32u) s_nopen = 0u;
     if (OBS && tid < 2u) s_obs[tid] = 0u;
-    if (OBS) __syncthreads();
     uint32_t o_neq = 0u, o_one = 0u;
     (void)o_neq; (void)o_one; (void)s_obs;
+    if (tid == 0u) {                 // after griddepcontrol.wait: the spins of S^t are complete
+        mbar_arrive_expect_tx(&s_bar, (uint32_t)TILE_SITES);
+        tma_load_2d(s_ew, &spin_map, x0, y0, &s_bar);
+    }
     if (MODEL == 1) {
         for (uint32_t k = tid; k < q2 * q2; k += TILE_THREADS) s_table[k] = md.table[k];
         m = axis_of_sweep(key, t, (uint32_t)md.q);
-        __syncthreads();
     }
 
     // ---------------- phase A: bonds of rows 8 warp .. 8 warp + 7, four sites per lane ----------------------
@@ -229,12 +274,20 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, uint16_t
         const uint32_t nth = 0u - md.thr_potts;                           // 2^32 - threshold (mod 2^32)
         const uint32_t emask = md.thr_potts ? 0x80808080u : 0u;           // threshold 0: no bond at all
         (void)nth; (void)emask;
+        // halo first (plain loads, in flight together with the box): the column right of the tile for lane 31, the row
+        // below the tile for the last warp
+#pragma unroll
+        for (int j = 0; j < ROWS_PER_WARP; ++j) hal[j] = (lane == 31u) ? (uint32_t)spins[(size_t)(y0 + ly0 + j) * L + xr] : 0u;
+        row[ROWS_PER_WARP] = 0u;
+        if (ly0 + ROWS_PER_WARP == (uint32_t)TH) {
+            const uint32_t gy = (y0 + TH == L) ? 0u : y0 + TH;
+            row[ROWS_PER_WARP] = *reinterpret_cast<const uint32_t *>(spins + (size_t)gy * L + gx);
+        }
+        __syncthreads();             // the mbarrier is initialised (thread 0, first statement), s_table / s_obs are written
+        mbar_wait(&s_bar, 0u);       // the box has landed
 #pragma unroll
         for (int j = 0; j <= ROWS_PER_WARP; ++j) {
-            uint32_t gy = y0 + ly0 + j;
-            if (gy == L) gy = 0u;
-            row[j] = *reinterpret_cast<const uint32_t *>(spins + (size_t)gy * L + gx);
-            if (j < ROWS_PER_WARP) hal[j] = (lane == 31u) ? (uint32_t)spins[(size_t)gy * L + xr] : 0u;
+            if (ly0 + (uint32_t)j < (uint32_t)TH) row[j] = s_ew[(ly0 + (uint32_t)j) * (TW / 4) + lane];
             if (MODEL == 1) {
                 // clock: work on c = (2 s - m) mod 2q from here on (R4), four bytes at a time
                 row[j] = clock_c4(row[j], m, q2);
@@ -850,10 +903,39 @@ __global__ void k_resolve_labels(Model md, const uint16_t *lab16, const unsigned
 // ---------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------
-static inline int tiled_init(TiledState &st, const Model &md, char *ws)
+// Tensor map of one [L][L] uint8 spin buffer with a TW x TH box (no swizzle, no interleave).  The driver's encoder is
+// reached through the runtime (no link against libcuda).
+static inline int make_spin_map(CUtensorMap *map, const uint8_t *base, int L)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+            qres != cudaDriverEntryPointSuccess)
+            return -1;
+        encode = reinterpret_cast<encode_fn>(fn);
+    }
+    const cuuint64_t dims[2] = { (cuuint64_t)L, (cuuint64_t)L };      // innermost first
+    const cuuint64_t strides[1] = { (cuuint64_t)L };                  // bytes between rows
+    const cuuint32_t box[2] = { (cuuint32_t)TW, (cuuint32_t)TH };
+    const cuuint32_t estr[2] = { 1u, 1u };
+    const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2u, const_cast<uint8_t *>(base), dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? 0 : -1;
+}
+
+static inline int tiled_init(TiledState &st, const Model &md, char *ws, const uint8_t *spins_a, const uint8_t *spins_b)
 {
     const size_t L = (size_t)md.L;
     st.L = md.L;
+    st.map_base[0] = spins_a;
+    st.map_base[1] = spins_b;
+    if (make_spin_map(&st.map[0], spins_a, md.L) != 0 || make_spin_map(&st.map[1], spins_b, md.L) != 0) return -1;
     size_t off = 0;
     st.lab16 = reinterpret_cast<uint16_t *>(ws);
     off += (2 * L * L + 1023) / 1024 * 1024;
@@ -880,14 +962,18 @@ static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, co
         cudaFuncSetAttribute(k_tile_label<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
         cudaFuncSetAttribute(k_tile_label<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
     }
+    const int which = in == st.map_base[0] ? 0 : in == st.map_base[1] ? 1 : -1;
+    if (which < 0) return cudaErrorInvalidValue;     // a spin buffer without a tensor map
+    const CUtensorMap &tm = st.map[which];
+    unsigned long long *const none = nullptr;
     if (md.model == 0 && md.q == 2 && obs)
-        return launch_pdl(k_tile_label<0, true>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge,
+        return launch_pdl(k_tile_label<0, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge, st.vedge,
                           st.edges, st.ocount, fuse, stats, obs);
     if (md.model == 0)
-        return launch_pdl(k_tile_label<0, false>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge,
-                          st.edges, st.ocount, fuse, stats, (unsigned long long *)nullptr);
-    return launch_pdl(k_tile_label<1, false>, tiles, TILE_THREADS, stream, md, key, t, in, st.lab16, parent, st.hedge, st.vedge, st.edges,
-                      st.ocount, fuse, stats, (unsigned long long *)nullptr);
+        return launch_pdl(k_tile_label<0, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge, st.vedge,
+                          st.edges, st.ocount, fuse, stats, none);
+    return launch_pdl(k_tile_label<1, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge, st.vedge,
+                      st.edges, st.ocount, fuse, stats, none);
 }
 
 // One sweep: in = S^t (left untouched), out = S^{t+1}.  ev (optional): ev[0] is recorded before the first kernel,
