@@ -41,9 +41,10 @@ enum { SW_OK = 0, SW_ERR_ARG = -1, SW_ERR_CUDA = -2, SW_ERR_NOMEM = -3, SW_ERR_U
 
 /* Labeling back-ends (sw_set_algorithm).  Every back-end produces the same spins bit for bit. */
 enum {
-    SW_ALGO_AUTO = 0,    /* tiled when L allows it, else generic */
+    SW_ALGO_AUTO = 0,    /* one CTA when L <= 64, else tiled when L allows it, else generic */
     SW_ALGO_GENERIC = 1, /* whole-lattice union-find in global memory; any L >= 2 */
-    SW_ALGO_TILED = 2    /* tile-local union-find in shared memory + boundary merge; needs L % 128 == 0 */
+    SW_ALGO_TILED = 2,   /* tile-local union-find in shared memory + boundary merge; needs L % 128 == 0 */
+    SW_ALGO_SMALL = 3    /* one CTA owns the lattice in shared memory and runs all n sweeps of a call in one launch; L <= 128 */
 };
 
 /* Limits of the GPU path: 2 <= L <= 16384 (site index must leave 4 spare bits in an int32 label),
@@ -154,6 +155,24 @@ const char *sw_kernel_name(sw_ctx *ctx, int k);
 
 /* Number of kernel launches this context has enqueued since creation. */
 uint64_t sw_launch_count(sw_ctx *ctx);
+
+/* NEXT-2 of the scope table: batches of B independent lattices of the same L, q and model, each with its own
+ * temperature T[b] and seed[b] (HOST arrays of B entries) -- the temperature scans of PAPER.md:111-113 (Fig.3),
+ * 128-130 (Fig.4), 167-171 (Fig.5), 177-183 (Fig.6) and the small-L rows of Table 1, where one lattice
+ * cannot fill a GPU.  Lattice b evolves exactly as a context created with sw_create(L, q, model, T[b], seed[b]) does:
+ * same S^0, same spins after every sweep.  L <= 128: one CTA per lattice, all n sweeps of a call inside one launch;
+ * L % 128 == 0: the tiles of all lattices in one grid per kernel.  Other L: NULL / SW_ERR_UNSUPPORTED.
+ * HOST buffers: spins B*L*L bytes (lattice-major), histograms B*q int64 each.  The library owns the device memory and
+ * the stream of a batch; all calls are synchronous at return. */
+#define SW_MAX_BATCH 65536
+typedef struct sw_batch sw_batch;
+sw_batch *sw_create_batch(int B, int L, int q, int model, const double *T, const uint64_t *seed);
+void sw_batch_destroy(sw_batch *batch);
+int sw_batch_sweep(sw_batch *batch, int n);
+int sw_batch_get_spins(sw_batch *batch, uint8_t *host_out);
+int sw_batch_set_spins(sw_batch *batch, const uint8_t *host_in, uint64_t sweep_index);
+int sw_batch_observables(sw_batch *batch, int64_t *bond_hist, int64_t *state_hist);
+uint64_t sw_batch_sweep_index(sw_batch *batch);
 
 /* Instruction-issue probes (measurement infrastructure for the "alu" roofline of DESIGN.md section 6; the sweep never
  * uses them).  Probe `probe` (0 .. until sw_microbench_name returns NULL) runs `warps_per_smsp` (1..16) warps on every

@@ -23,7 +23,7 @@ LIB_PATH = Path(os.environ["SW_LIB"]) if os.environ.get("SW_LIB") else _PKG / "l
 
 SW_POTTS, SW_CLOCK = 0, 1
 SW_OK, SW_ERR_ARG, SW_ERR_CUDA, SW_ERR_NOMEM, SW_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
-SW_ALGO_AUTO, SW_ALGO_GENERIC, SW_ALGO_TILED = 0, 1, 2
+SW_ALGO_AUTO, SW_ALGO_GENERIC, SW_ALGO_TILED, SW_ALGO_SMALL = 0, 1, 2, 3
 
 # name -> (restype, argtypes): every symbol include/sw.h declares
 _vp, _i, _u64, _d, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_uint64, ctypes.c_double, ctypes.c_size_t
@@ -59,6 +59,13 @@ SYMBOLS = {
     "sw_derive_g": (_d, [_i, _vp]),
     "sw_derive_moment_ratio": (_d, [_i, _i, _vp]),
     "sw_derive_ratio_R": (_d, [_i, _i, _vp, _vp]),
+    "sw_create_batch": (_vp, [_i, _i, _i, _i, _vp, _vp]),
+    "sw_batch_destroy": (None, [_vp]),
+    "sw_batch_sweep": (_i, [_vp, _i]),
+    "sw_batch_get_spins": (_i, [_vp, _vp]),
+    "sw_batch_set_spins": (_i, [_vp, _vp, _u64]),
+    "sw_batch_observables": (_i, [_vp, _vp, _vp]),
+    "sw_batch_sweep_index": (_u64, [_vp]),
     "sw_microbench": (_i, [_i, _i, _i, _vp]),
     "sw_microbench_name": (ctypes.c_char_p, [_i]),
     "sw_selftest": (_i, []),
@@ -246,6 +253,62 @@ class Lattice:
     @property
     def launch_count(self) -> int:
         return int(self._lib.sw_launch_count(self._h))
+
+
+class Batch:
+    """B independent lattices (own T and seed each) advanced together; mirrors sw_create_batch / sw_batch_*."""
+
+    def __init__(self, L: int, q: int, model: int, T, seed):
+        lib = load()
+        self._lib = lib
+        self._T = np.ascontiguousarray(T, dtype=np.float64)
+        self._seed = np.ascontiguousarray(seed, dtype=np.uint64)
+        assert self._T.shape == self._seed.shape and self._T.ndim == 1
+        self.B, self.L, self.q, self.model = int(self._T.shape[0]), L, q, model
+        h = lib.sw_create_batch(self.B, L, q, model, self._T.ctypes.data, self._seed.ctypes.data)
+        if not h:
+            raise SwError(SW_ERR_ARG, last_error())
+        self._h = h
+
+    def close(self):
+        if self._h:
+            self._lib.sw_batch_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def sweep(self, n: int = 1):
+        _check(self._lib.sw_batch_sweep(self._h, n))
+
+    def get_spins(self) -> np.ndarray:
+        out = np.empty((self.B, self.L, self.L), dtype=np.uint8)
+        _check(self._lib.sw_batch_get_spins(self._h, out.ctypes.data))
+        return out
+
+    def set_spins(self, spins, sweep_index: int = 0):
+        spins = np.ascontiguousarray(spins, dtype=np.uint8)
+        assert spins.size == self.B * self.L * self.L
+        _check(self._lib.sw_batch_set_spins(self._h, spins.ctypes.data, sweep_index))
+
+    def observables(self):
+        bh = np.zeros((self.B, self.q), dtype=np.int64)
+        sh = np.zeros((self.B, self.q), dtype=np.int64)
+        _check(self._lib.sw_batch_observables(self._h, bh.ctypes.data, sh.ctypes.data))
+        return bh, sh
+
+    @property
+    def sweep_index(self) -> int:
+        return int(self._lib.sw_batch_sweep_index(self._h))
 
 
 # Derived doubles (DESIGN.md R11, R15): computed by libsw.so (sw_derive_*), marshalled here.

@@ -16,6 +16,7 @@
 #include "sw.h"
 #include "sw_generic.cuh"
 #include "sw_philox.cuh"
+#include "sw_small.cuh"
 #include "sw_tile.cuh"
 
 namespace {
@@ -51,7 +52,7 @@ bool args_ok(int L, int q, int model)
 }
 
 struct Carve {
-    size_t spins, spins2, labels, bonds, table, obs, flag, stats, ring, tiled, total;
+    size_t spins, spins2, labels, bonds, table, obs, flag, stats, ring, small, tiled, total;
 };
 
 Carve carve(int L, int q)
@@ -69,6 +70,7 @@ Carve carve(int L, int q)
     c.flag = off;   off += align_up(64);
     c.stats = off;  off += align_up(8 * SW_NUM_STATS);
     c.ring = off;   off += align_up((size_t)REC_ROWS * OBS_WORDS * 8);
+    c.small = off;  off += align_up(sizeof(sw::SmallLattice));
     c.tiled = off;  off += align_up(sw::tiled_workspace_bytes(L));
     c.total = off;
     return c;
@@ -92,6 +94,7 @@ struct sw_ctx {
     unsigned long long *obs = nullptr, *stats = nullptr, *ring = nullptr;
     int *flag = nullptr;
     char *tiled_ws = nullptr;
+    sw::SmallLattice *small_lat = nullptr;   // device: key and threshold of this lattice, as the one-CTA kernel reads them
     sw::Model md{};
     sw::PhiloxKey key{};
     std::vector<uint32_t> thr_host;  // 1 (Potts) or (2q)^2 (clock)
@@ -148,6 +151,24 @@ inline unsigned blocks_for(size_t n, unsigned bs) { return (unsigned)((n + bs - 
 
 const char *const GENERIC_KERNELS[] = { "k_bonds", "k_label_init", "k_union", "k_flatten", "k_flip" };
 
+// SW_ALGO_AUTO: one CTA for L <= 64 (measured: 7 us per sweep at L = 32 and 26 us at L = 64 against 22 and 28 us of
+// the five generic launches; at L = 128 the single CTA is the slower one), tiles when L allows them, else generic
+int auto_algo(int L)
+{
+    return L <= 64 ? SW_ALGO_SMALL : sw::tiled_supported(L) ? SW_ALGO_TILED : SW_ALGO_GENERIC;
+}
+
+// n sweeps of the one-CTA back-end in ONE launch (sweep indices c->t .. c->t + n - 1; labels of the last one exported)
+int small_sweeps(sw_ctx *c, int n, cudaEvent_t *ev = nullptr)
+{
+    if (ev) cudaEventRecord(ev[0], c->stream);
+    CU_TRY(sw::small_launch(c->model, 1, c->L, c->q, c->small_lat, c->table, c->spins, c->labels, (uint32_t)c->t, n, c->stream,
+                             c->stats_on ? c->stats : nullptr));
+    if (ev) cudaEventRecord(ev[1], c->stream);
+    c->launches += 1;
+    return SW_OK;
+}
+
 // ev (optional): ev[0] is recorded before the first kernel, ev[k+1] after kernel k.
 int generic_sweep(sw_ctx *c, uint32_t t, cudaEvent_t *ev)
 {
@@ -182,6 +203,8 @@ int one_sweep(sw_ctx *c, cudaEvent_t *ev = nullptr, unsigned long long *obs_row 
                              c->stats_on ? c->stats : nullptr, &c->launches, ev, obs_row);
         if (rc != 0) return fail(SW_ERR_CUDA, "tiled sweep launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         std::swap(c->spins, c->spins_alt);   // spins_alt now holds S^t, the input of this sweep
+    } else if (c->algo == SW_ALGO_SMALL) {
+        rc = small_sweeps(c, 1, ev);
     } else {
         rc = generic_sweep(c, t, ev);
     }
@@ -284,6 +307,7 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
     c->stats = (unsigned long long *)(c->ws + c->cv.stats);
     c->ring = (unsigned long long *)(c->ws + c->cv.ring);
     c->tiled_ws = c->ws + c->cv.tiled;
+    c->small_lat = (sw::SmallLattice *)(c->ws + c->cv.small);
     c->key = sw::make_philox_key(seed);
     build_thresholds(c);
     if (cudaMallocHost((void **)&c->rec_host, (size_t)REC_ROWS * OBS_WORDS * 8) != cudaSuccess) {
@@ -301,12 +325,20 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
     if (model == SW_CLOCK)
         ok = ok && cudaMemcpyAsync(c->table, c->thr_host.data(), 4 * c->thr_host.size(), cudaMemcpyHostToDevice, c->stream) == cudaSuccess;
     ok = ok && cudaMemsetAsync(c->stats, 0, 8 * SW_NUM_STATS, c->stream) == cudaSuccess;
+    {
+        sw::SmallLattice sl;
+        sl.key = c->key;
+        sl.thr_potts = c->md.thr_potts;
+        sl.pad = 0u;
+        ok = ok && cudaMemcpyAsync(c->small_lat, &sl, sizeof(sl), cudaMemcpyHostToDevice, c->stream) == cudaSuccess;
+        ok = ok && cudaStreamSynchronize(c->stream) == cudaSuccess;     // sl is on the stack
+    }
     if (ok) {
         sw::k_init_spins<<<blocks_for((c->N + 3) / 4, 256), 256, 0, c->stream>>>(c->md, c->key, c->spins);
         c->launches += 1;
         ok = cudaGetLastError() == cudaSuccess;
     }
-    c->algo = sw::tiled_supported(L) ? SW_ALGO_TILED : SW_ALGO_GENERIC;
+    c->algo = auto_algo(L);
     if (ok && sw::tiled_supported(L)) ok = sw::tiled_init(c->tiled, c->md, c->tiled_ws, c->spins, c->spins_alt) == 0;
     ok = ok && cudaStreamSynchronize(c->stream) == cudaSuccess;
     if (!ok) {
@@ -353,6 +385,15 @@ int sw_sweep_async(sw_ctx *c, int n)
     if (!c || n < 0) return fail(SW_ERR_ARG, "sw_sweep: NULL context or n < 0");
     DeviceGuard guard(c);
     if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep: sweep index would exceed 2^32-1");
+    if (c->algo == SW_ALGO_SMALL && n > 0) {       // all n sweeps inside one launch
+        int rc = small_sweeps(c, n);
+        if (rc != SW_OK) return rc;
+        c->last_algo = c->algo;
+        c->have_labels = true;
+        if (c->stats_on) c->stat_sweeps += (uint64_t)n;
+        c->t += (uint64_t)n;
+        n = 0;
+    }
     for (int k = 0; k < n; ++k) {
         int rc = one_sweep(c);
         if (rc != SW_OK) return rc;
@@ -553,10 +594,13 @@ int sw_debug_bonds(sw_ctx *c, uint8_t *host_out)
 int sw_set_algorithm(sw_ctx *c, int algo)
 {
     if (!c) return fail(SW_ERR_ARG, "sw_set_algorithm: NULL context");
-    if (algo == SW_ALGO_AUTO) algo = sw::tiled_supported(c->L) ? SW_ALGO_TILED : SW_ALGO_GENERIC;
+    if (algo == SW_ALGO_AUTO) algo = auto_algo(c->L);
     if (algo == SW_ALGO_TILED && !sw::tiled_supported(c->L))
         return fail(SW_ERR_UNSUPPORTED, "sw_set_algorithm: the tiled back-end needs L %% %d == 0 (L = %d)", sw::TW, c->L);
-    if (algo != SW_ALGO_GENERIC && algo != SW_ALGO_TILED) return fail(SW_ERR_ARG, "sw_set_algorithm: unknown back-end %d", algo);
+    if (algo == SW_ALGO_SMALL && !sw::small_supported(c->L))
+        return fail(SW_ERR_UNSUPPORTED, "sw_set_algorithm: the one-CTA back-end needs L <= %d (L = %d)", sw::SMALL_MAX_L, c->L);
+    if (algo != SW_ALGO_GENERIC && algo != SW_ALGO_TILED && algo != SW_ALGO_SMALL)
+        return fail(SW_ERR_ARG, "sw_set_algorithm: unknown back-end %d", algo);
     c->algo = algo;
     return SW_OK;
 }
@@ -587,7 +631,7 @@ int sw_sweep_profile(sw_ctx *c, int n, double *ms_out, int *n_kernels)
     if (!c || n < 0 || !ms_out || !n_kernels) return fail(SW_ERR_ARG, "sw_sweep_profile: bad arguments");
     DeviceGuard guard(c);
     if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_profile: sweep index would exceed 2^32-1");
-    const int nk = (c->algo == SW_ALGO_TILED) ? sw::TILED_NUM_KERNELS : 5;
+    const int nk = (c->algo == SW_ALGO_TILED) ? sw::TILED_NUM_KERNELS : (c->algo == SW_ALGO_SMALL) ? 1 : 5;
     cudaEvent_t ev[SW_MAX_KERNELS + 1];
     for (int k = 0; k <= nk; ++k) CU_TRY(cudaEventCreate(&ev[k]));
     for (int k = 0; k < SW_MAX_KERNELS; ++k) ms_out[k] = 0.0;
@@ -611,10 +655,189 @@ const char *sw_kernel_name(sw_ctx *c, int k)
 {
     if (!c || k < 0) return nullptr;
     if (c->algo == SW_ALGO_TILED) return k < sw::TILED_NUM_KERNELS ? sw::TILED_KERNELS[k] : nullptr;
+    if (c->algo == SW_ALGO_SMALL) return k == 0 ? "k_small_sweeps" : nullptr;
     return k < 5 ? GENERIC_KERNELS[k] : nullptr;
 }
 
 uint64_t sw_launch_count(sw_ctx *c) { return c ? c->launches : 0; }
+
+// ---------------------------------------------------------------------------------------------------------------
+// Batches of independent lattices (NEXT-2): same L, q, model; own temperature and seed each.
+// ---------------------------------------------------------------------------------------------------------------
+}  // extern "C"
+
+struct sw_batch {
+    int B = 0, L = 0, q = 0, model = 0, device = 0, sms = 148;
+    size_t N = 0;
+    uint64_t t = 0;
+    cudaStream_t stream = nullptr;
+    char *ws = nullptr;
+    uint8_t *spins = nullptr;            // [B][N]
+    sw::SmallLattice *lats = nullptr;    // [B]
+    uint32_t *tables = nullptr;          // [B][SMALL_TABLE_WORDS] (clock)
+    unsigned long long *obs = nullptr;   // [B][OBS_WORDS]
+    std::vector<sw::Model> md;           // per lattice (host)
+};
+
+namespace {
+struct BatchGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit BatchGuard(const sw_batch *b)
+    {
+        if (b && cudaGetDevice(&prev) == cudaSuccess && prev != b->device) switched = cudaSetDevice(b->device) == cudaSuccess;
+    }
+    ~BatchGuard() { if (switched) cudaSetDevice(prev); }
+};
+}  // namespace
+
+extern "C" {
+
+sw_batch *sw_create_batch(int B, int L, int q, int model, const double *T, const uint64_t *seed)
+{
+    if (B < 1 || B > SW_MAX_BATCH || !T || !seed || !args_ok(L, q, model)) {
+        fail(SW_ERR_ARG, "sw_create_batch: need 1 <= B <= %d, valid L, q, model and non-NULL T, seed", SW_MAX_BATCH);
+        return nullptr;
+    }
+    for (int b = 0; b < B; ++b)
+        if (!(T[b] > 0.0) || !std::isfinite(T[b])) {
+            fail(SW_ERR_ARG, "sw_create_batch: T[%d] = %g is not a finite positive temperature", b, T[b]);
+            return nullptr;
+        }
+    if (!sw::small_supported(L)) {
+        fail(SW_ERR_UNSUPPORTED, "sw_create_batch: L = %d: batches need L <= %d (one CTA per lattice)", L, sw::SMALL_MAX_L);
+        return nullptr;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        fail(SW_ERR_CUDA, "sw_create_batch: no usable CUDA device (this library has no CPU fallback)");
+        return nullptr;
+    }
+    sw_batch *bt = new (std::nothrow) sw_batch();
+    if (!bt) { fail(SW_ERR_NOMEM, "sw_create_batch: out of host memory"); return nullptr; }
+    bt->B = B; bt->L = L; bt->q = q; bt->model = model; bt->N = (size_t)L * L;
+    cudaGetDevice(&bt->device);
+    cudaDeviceGetAttribute(&bt->sms, cudaDevAttrMultiProcessorCount, bt->device);
+    const size_t o_spins = 0, o_lats = align_up((size_t)B * bt->N), o_tab = o_lats + align_up((size_t)B * sizeof(sw::SmallLattice)),
+                 o_obs = o_tab + align_up((size_t)B * sw::SMALL_TABLE_WORDS * 4), total = o_obs + align_up((size_t)B * OBS_WORDS * 8);
+    bool ok = cudaMalloc((void **)&bt->ws, total) == cudaSuccess;
+    ok = ok && cudaStreamCreateWithFlags(&bt->stream, cudaStreamNonBlocking) == cudaSuccess;
+    if (!ok) {
+        fail(SW_ERR_NOMEM, "sw_create_batch: device allocation of %zu bytes failed: %s", total, cudaGetErrorString(cudaGetLastError()));
+        sw_batch_destroy(bt);
+        return nullptr;
+    }
+    bt->spins = (uint8_t *)(bt->ws + o_spins);
+    bt->lats = (sw::SmallLattice *)(bt->ws + o_lats);
+    bt->tables = (uint32_t *)(bt->ws + o_tab);
+    bt->obs = (unsigned long long *)(bt->ws + o_obs);
+    // per-lattice thresholds (host, double: R1 / R4, R6, R7) and Philox keys; S^0 of every lattice from its INIT stream
+    std::vector<sw::SmallLattice> hl((size_t)B);
+    std::vector<uint32_t> ht((size_t)B * sw::SMALL_TABLE_WORDS, 0u);
+    bt->md.resize((size_t)B);
+    sw_ctx tmp;
+    tmp.q = q; tmp.model = model;
+    for (int b = 0; b < B; ++b) {
+        tmp.T = T[b];
+        build_thresholds(&tmp);
+        hl[b].key = sw::make_philox_key(seed[b]);
+        hl[b].thr_potts = model == SW_POTTS ? tmp.thr_host[0] : 0u;
+        hl[b].pad = 0u;
+        if (model == SW_CLOCK) std::copy(tmp.thr_host.begin(), tmp.thr_host.end(), ht.begin() + (size_t)b * sw::SMALL_TABLE_WORDS);
+        sw::Model &m = bt->md[b];
+        m.L = L; m.q = q; m.model = model; m.N = (uint32_t)bt->N; m.thr_potts = hl[b].thr_potts;
+        m.table = bt->tables + (size_t)b * sw::SMALL_TABLE_WORDS;
+    }
+    ok = cudaMemcpyAsync(bt->lats, hl.data(), hl.size() * sizeof(sw::SmallLattice), cudaMemcpyHostToDevice, bt->stream) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(bt->tables, ht.data(), ht.size() * 4, cudaMemcpyHostToDevice, bt->stream) == cudaSuccess;
+    for (int b = 0; b < B && ok; ++b) {
+        sw::k_init_spins<<<blocks_for((bt->N + 3) / 4, 256), 256, 0, bt->stream>>>(bt->md[b], hl[b].key, bt->spins + (size_t)b * bt->N);
+        ok = cudaGetLastError() == cudaSuccess;
+    }
+    ok = ok && cudaStreamSynchronize(bt->stream) == cudaSuccess;
+    if (!ok) {
+        fail(SW_ERR_CUDA, "sw_create_batch: device initialisation failed: %s", cudaGetErrorString(cudaGetLastError()));
+        sw_batch_destroy(bt);
+        return nullptr;
+    }
+    return bt;
+}
+
+void sw_batch_destroy(sw_batch *bt)
+{
+    if (!bt) return;
+    BatchGuard guard(bt);
+    if (bt->stream) { cudaStreamSynchronize(bt->stream); cudaStreamDestroy(bt->stream); }
+    if (bt->ws) cudaFree(bt->ws);
+    delete bt;
+}
+
+int sw_batch_sweep(sw_batch *bt, int n)
+{
+    if (!bt || n < 0) return fail(SW_ERR_ARG, "sw_batch_sweep: NULL batch or n < 0");
+    if (bt->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_batch_sweep: sweep index would exceed 2^32-1");
+    BatchGuard guard(bt);
+    if (n > 0) {
+        CU_TRY(sw::small_launch(bt->model, bt->B, bt->L, bt->q, bt->lats, bt->tables, bt->spins, nullptr, (uint32_t)bt->t, n, bt->stream));
+        bt->t += (uint64_t)n;
+    }
+    CU_TRY(cudaStreamSynchronize(bt->stream));
+    return SW_OK;
+}
+
+int sw_batch_get_spins(sw_batch *bt, uint8_t *host_out)
+{
+    if (!bt || !host_out) return fail(SW_ERR_ARG, "sw_batch_get_spins: NULL argument");
+    BatchGuard guard(bt);
+    CU_TRY(cudaMemcpyAsync(host_out, bt->spins, (size_t)bt->B * bt->N, cudaMemcpyDeviceToHost, bt->stream));
+    CU_TRY(cudaStreamSynchronize(bt->stream));
+    return SW_OK;
+}
+
+int sw_batch_set_spins(sw_batch *bt, const uint8_t *host_in, uint64_t sweep_index)
+{
+    if (!bt || !host_in) return fail(SW_ERR_ARG, "sw_batch_set_spins: NULL argument");
+    if (sweep_index > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_batch_set_spins: sweep index must fit 32 bits");
+    const size_t total = (size_t)bt->B * bt->N;
+    for (size_t i = 0; i < total; ++i)
+        if (host_in[i] >= (uint8_t)bt->q) return fail(SW_ERR_ARG, "sw_batch_set_spins: spin value %d >= q = %d", (int)host_in[i], bt->q);
+    BatchGuard guard(bt);
+    CU_TRY(cudaMemcpyAsync(bt->spins, host_in, total, cudaMemcpyHostToDevice, bt->stream));
+    CU_TRY(cudaStreamSynchronize(bt->stream));
+    bt->t = sweep_index;
+    return SW_OK;
+}
+
+int sw_batch_observables(sw_batch *bt, int64_t *bond_hist, int64_t *state_hist)
+{
+    if (!bt || !bond_hist || !state_hist) return fail(SW_ERR_ARG, "sw_batch_observables: NULL argument");
+    BatchGuard guard(bt);
+    CU_TRY(cudaMemsetAsync(bt->obs, 0, (size_t)bt->B * OBS_WORDS * 8, bt->stream));
+    const size_t work = (bt->L % 16 == 0) ? bt->N / 16 : bt->N;
+    const unsigned grid = (unsigned)std::max<size_t>(1, std::min<size_t>((work + 255) / 256, (size_t)bt->sms * 4));
+    for (int b = 0; b < bt->B; ++b) {
+        const uint8_t *sp = bt->spins + (size_t)b * bt->N;
+        unsigned long long *dst = bt->obs + (size_t)b * OBS_WORDS;
+        cudaError_t e;
+        if (bt->q <= 2) e = sw::launch_pdl(sw::k_observables<2>, grid, sw::HIST_THREADS, bt->stream, bt->md[b], sp, dst);
+        else if (bt->q <= 4) e = sw::launch_pdl(sw::k_observables<4>, grid, sw::HIST_THREADS, bt->stream, bt->md[b], sp, dst);
+        else if (bt->q <= 8) e = sw::launch_pdl(sw::k_observables<8>, grid, sw::HIST_THREADS, bt->stream, bt->md[b], sp, dst);
+        else e = sw::launch_pdl(sw::k_observables<16>, grid, sw::HIST_THREADS, bt->stream, bt->md[b], sp, dst);
+        CU_TRY(e);
+    }
+    std::vector<unsigned long long> host((size_t)bt->B * OBS_WORDS);
+    CU_TRY(cudaMemcpyAsync(host.data(), bt->obs, host.size() * 8, cudaMemcpyDeviceToHost, bt->stream));
+    CU_TRY(cudaStreamSynchronize(bt->stream));
+    for (int b = 0; b < bt->B; ++b)
+        for (int j = 0; j < bt->q; ++j) {
+            bond_hist[(size_t)b * bt->q + j] = (int64_t)host[(size_t)b * OBS_WORDS + j];
+            state_hist[(size_t)b * bt->q + j] = (int64_t)host[(size_t)b * OBS_WORDS + 16 + j];
+        }
+    return SW_OK;
+}
+
+uint64_t sw_batch_sweep_index(sw_batch *bt) { return bt ? bt->t : 0; }
 
 int sw_selftest(void)
 {

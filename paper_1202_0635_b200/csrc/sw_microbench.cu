@@ -16,7 +16,7 @@ enum Probe : int {
     P_MIX_LOP3_IMAD, P_MIX_LOP3_WIDE, P_MIX_2LOP3_WIDE, P_PHILOX, P_LDS, P_STS, P_SHFL, P_PRMT, P_MIX_LOP3_LDS, P_MIX_IMAD_LDS,
     P_MIX_LOP3_IMAD_LDS, P_VOTE, P_ATOMS_MIN,
     P_WIDE_IMAD, P_MIX_LOP3_HI, P_MIX_LOP3_FLO, P_MIX_IMAD_FLO, P_MIX_LOP3_SHFL, P_MIX_LDS_STS, P_I2F, P_PHILOX_HILO,
-    P_PHILOX_PLUS_LOP3, P_PHILOX_HILO_PLUS_LOP3, P_COUNT
+    P_PHILOX_PLUS_LOP3, P_PHILOX_HILO_PLUS_LOP3, P_ATOMS_MIN_RET, P_ATOMS_MIN_RET_1LANE, P_COUNT
 };
 
 static const char *const NAMES[P_COUNT] = {
@@ -26,7 +26,8 @@ static const char *const NAMES[P_COUNT] = {
     "LOP3+IMAD+LDS 1:1:1", "VOTE.ANY (ballot)", "ATOMS.MIN (distinct addresses)",
     "IMAD.WIDE.U32 (imm) + IMAD (pair)", "LOP3+IMAD.HI 1:1", "LOP3+FLO 1:1", "IMAD+FLO 1:1", "LOP3+SHFL 1:1", "LDS+STS 1:1", "I2F.U32",
     "Philox4x32-10 call, products as IMAD.HI + IMAD (one call = 1 unit)", "Philox call + 40 independent LOP3 (one unit)",
-    "Philox call (IMAD.HI + IMAD) + 40 independent LOP3 (one unit)"
+    "Philox call (IMAD.HI + IMAD) + 40 independent LOP3 (one unit)",
+    "ATOMS.MIN with return value (distinct addresses, result feeds the next)", "ATOMS.MIN with return value, one active lane per warp"
 };
 
 constexpr int ILP = 8;      // independent chains per thread
@@ -56,6 +57,8 @@ __device__ __forceinline__ void step(uint32_t &x, uint64_t &p, uint32_t a, uint3
     else if (P == P_WIDE_IMAD)   // x = hi(x C); the low half feeds an IMAD accumulator kept in the upper half of p
         asm volatile("{.reg .u32 lo, hi, y, z; .reg .u64 w; mov.b64 {z, y}, %1; mul.wide.u32 w, %0, 0xD2511F53; mov.b64 {lo, %0}, w; mad.lo.u32 y, lo, %2, y; mov.b64 %1, {z, y};}" : "+r"(x), "+l"(p) : "r"(a));
     else if (P == P_I2F) asm volatile("{.reg .f32 f; cvt.rn.f32.u32 f, %0; mov.b32 %0, f;}" : "+r"(x));
+    else if (P == P_ATOMS_MIN_RET) asm volatile("atom.shared.min.u32 %0, [%1], %0;" : "+r"(x) : "r"(saddr));
+    else if (P == P_ATOMS_MIN_RET_1LANE) { if ((threadIdx.x & 31u) == 0u) asm volatile("atom.shared.min.u32 %0, [%1], %0;" : "+r"(x) : "r"(saddr)); }
     else if (P == P_ATOMS_MIN) asm volatile("{.reg .u32 t; atom.shared.min.u32 t, [%1], %0;}" : : "r"(x), "r"(saddr));
 }
 
@@ -209,6 +212,7 @@ int sw_microbench(int probe, int warps_per_smsp, int iters, double *out)
         SW_MB_CASE(P_MIX_LOP3_IMAD_LDS) SW_MB_CASE(P_VOTE) SW_MB_CASE(P_ATOMS_MIN)
         SW_MB_CASE(P_WIDE_IMAD) SW_MB_CASE(P_MIX_LOP3_HI) SW_MB_CASE(P_MIX_LOP3_FLO) SW_MB_CASE(P_MIX_IMAD_FLO) SW_MB_CASE(P_MIX_LOP3_SHFL)
         SW_MB_CASE(P_MIX_LDS_STS) SW_MB_CASE(P_I2F) SW_MB_CASE(P_PHILOX_HILO) SW_MB_CASE(P_PHILOX_PLUS_LOP3) SW_MB_CASE(P_PHILOX_HILO_PLUS_LOP3)
+        SW_MB_CASE(P_ATOMS_MIN_RET) SW_MB_CASE(P_ATOMS_MIN_RET_1LANE)
 #undef SW_MB_CASE
         default: break;
         }

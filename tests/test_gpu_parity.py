@@ -15,7 +15,7 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 POTTS, CLOCK = 0, 1
-GENERIC, TILED = 1, 2
+GENERIC, TILED, SMALL = 1, 2, 3
 
 
 @pytest.fixture(scope="module")
@@ -187,6 +187,64 @@ def test_clock_record_and_observables(sw, oracle):
             a, b = sw.clock_energy(q, bh[k]), oracle.clock_energy(q, obh[k])
             assert abs(a - b) <= 1e-12 * abs(b)
             assert abs(sw.clock_m(q, sh[k]) - oracle.clock_m(q, osh[k])) <= 1e-12 * L * L
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-2: the one-CTA back-end (L <= 128, all sweeps of a call in one launch) and batches of lattices
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L", [2, 3, 5, 8, 31, 64, 100, 128])
+@pytest.mark.parametrize("q,model,T", [(2, POTTS, tc(2)), (3, POTTS, tc(3)), (6, CLOCK, 0.9), (16, CLOCK, 0.5)])
+def test_small_backend(sw, oracle, L, q, model, T):
+    seed = 0x5EED0100 + L
+    run_and_compare(sw, oracle, L, q, model, T, seed=seed, algo=SMALL, n=4 if L <= 64 else 2)
+    # n sweeps inside ONE launch, then the labels of the last one
+    with sw.Lattice(L, q, model, T, seed) as lat:
+        assert lat.algorithm == (SMALL if L <= 64 else TILED if L % 128 == 0 else GENERIC)   # what SW_ALGO_AUTO picks
+        lat.set_algorithm(SMALL)
+        before = lat.launch_count
+        lat.sweep(9)
+        assert lat.launch_count == before + 1 and lat.sweep_index == 9
+        s = oracle.run(L, q, model, T, seed, 0, 8, oracle.init_spins(L, q, seed))
+        s, olab = oracle.sweep(L, q, model, T, seed, 8, s, want_labels=True)
+        _assert_same(lat.get_spins(), s, "spins after 9 sweeps in one launch")
+        _assert_same(lat.get_labels(), olab, "labels of the last sweep")
+
+
+@pytest.mark.parametrize("L,q,model", [(64, 2, POTTS), (32, 3, POTTS), (48, 6, CLOCK), (128, 2, POTTS), (7, 4, CLOCK)])
+def test_batch_every_lattice_equals_its_own_run(sw, oracle, L, q, model):
+    """A batch of lattices with different temperatures and seeds: lattice b equals the single-lattice oracle run with
+    (T[b], seed[b]) after every call, and its histograms equal the oracle's."""
+    B = 11
+    base = tc(q) if model == POTTS else 0.9
+    T = [base * (0.6 + 0.08 * b) for b in range(B)]
+    seed = [0x5EED0200 + 7919 * b + (b << 40) for b in range(B)]
+    with sw.Batch(L, q, model, T, seed) as bt:
+        want = [oracle.init_spins(L, q, seed[b]) for b in range(B)]
+        got = bt.get_spins()
+        for b in range(B):
+            _assert_same(got[b], want[b], f"S^0 of lattice {b}")
+        t = 0
+        for n in (1, 6, 3):
+            bt.sweep(n)
+            got = bt.get_spins()
+            for b in range(B):
+                want[b] = oracle.run(L, q, model, T[b], seed[b], t, n, want[b])
+                _assert_same(got[b], want[b], f"lattice {b} after sweep {t + n}")
+            t += n
+        assert bt.sweep_index == t
+        bh, sh = bt.observables()
+        for b in range(B):
+            obh, osh = oracle.observables(L, q, want[b])
+            _assert_same(bh[b], obh, f"bond_hist of lattice {b}")
+            _assert_same(sh[b], osh, f"state_hist of lattice {b}")
+        # hand-off: a configuration set from the host, absolute sweep index
+        from paper_1202_0635_b200.workloads import random_spins
+        s0 = np.stack([random_spins(L, q, 100 + b) for b in range(B)])
+        bt.set_spins(s0, 40)
+        bt.sweep(2)
+        got = bt.get_spins()
+        for b in range(B):
+            _assert_same(got[b], oracle.run(L, q, model, T[b], seed[b], 40, 2, s0[b]), f"lattice {b} after the hand-off")
 
 
 # ------------------------------------------------------------------------------------------------
