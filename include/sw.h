@@ -160,8 +160,8 @@ uint64_t sw_launch_count(sw_ctx *ctx);
  * temperature T[b] and seed[b] (HOST arrays of B entries) -- the temperature scans of PAPER.md:111-113 (Fig.3),
  * 128-130 (Fig.4), 167-171 (Fig.5), 177-183 (Fig.6) and the small-L rows of Table 1, where one lattice
  * cannot fill a GPU.  Lattice b evolves exactly as a context created with sw_create(L, q, model, T[b], seed[b]) does:
- * same S^0, same spins after every sweep.  L <= 128: one CTA per lattice, all n sweeps of a call inside one launch;
- * L % 128 == 0: the tiles of all lattices in one grid per kernel.  Other L: NULL / SW_ERR_UNSUPPORTED.
+ * same S^0, same spins after every sweep.  L % 128 == 0: the tiles of all lattices in one grid per kernel; other
+ * L <= 128: one CTA per lattice, all n sweeps of a call inside one launch.  Other L: NULL / SW_ERR_UNSUPPORTED.
  * HOST buffers: spins B*L*L bytes (lattice-major), histograms B*q int64 each.  The library owns the device memory and
  * the stream of a batch; all calls are synchronous at return. */
 #define SW_MAX_BATCH 65536

@@ -88,6 +88,16 @@ constexpr int OCAP = 512;               // open roots listed per tile (<= 128 + 
 static_assert(LAB_WORDS <= (int)LMASK + 1, "skewed local index must fit the label field");
 static_assert((TILE_THREADS / 32) * ROWS_PER_WARP == TH, "phase A row split");
 
+// Batches (NEXT-2): the tiles of B lattices of the same L, q, model in one grid.  Global tile g = lattice * tiles per
+// lattice + local tile; spins, labels and the seam masks of lattice b sit b strides further; the node, edge and
+// open-count arrays are indexed by the global tile, so they need no stride.  Key and thresholds differ per lattice.
+struct BatchView {
+    uint32_t tiles_per_lattice;
+    const PhiloxKey *keys;      // [B]
+    const uint32_t *thr;        // [B] Potts threshold
+    const uint32_t *tables;     // [B][(2*16)^2] clock tables
+};
+
 struct TiledState {
     uint16_t *lab16 = nullptr;   // [L][L] tile-local root of every site (+ LOPEN)
     uint32_t *hedge = nullptr;   // [L/128][L/32]  bit (y & 31) of word y >> 5: +x bond of column 128 tx + 127, row y
@@ -98,18 +108,16 @@ struct TiledState {
     // TMA: one tensor map per spin buffer of the ping-pong ([L][L] uint8, box = one 128 x 64 tile)
     const uint8_t *map_base[2] = { nullptr, nullptr };
     CUtensorMap map[2];
+    // batches: number of lattices in the arrays above, and where their keys / thresholds live
+    uint32_t nlat = 1;
+    bool batch = false;
+    BatchView bv{};
 };
 
 static inline bool tiled_supported(int L) { return L >= TW && L % TW == 0 && L % TH == 0; }
 
-static inline size_t tiled_workspace_bytes(int L)
-{
-    if (!tiled_supported(L)) return 0;
-    const size_t N = (size_t)L * L;
-    const size_t tiles = (size_t)(L / TW) * (L / TH);
-    return 2 * N + 1024 + (size_t)(L / TW) * (L / 32) * 4 + 1024 + (size_t)(L / TH) * (L / 32) * 4 + 1024 +
-           tiles * ECNT * 2 + 1024 + tiles * 4 + 1024;
-}
+static inline size_t tiled_workspace_bytes_n(int L, size_t nlat);
+static inline size_t tiled_workspace_bytes(int L) { return tiled_workspace_bytes_n(L, 1); }
 
 // ---- shared-memory union-find by minimum index (same scheme as uf_union in sw_generic.cuh) ------------------
 __device__ __forceinline__ uint32_t sfind_halve(volatile uint32_t *lab, uint32_t a)
@@ -207,11 +215,13 @@ __global__ void k_selftest_compare(const uint32_t *vals, int n, int *bad)
 // thread, completion on an mbarrier; it lands in the storage of the edge lists, which phase B only starts to use after
 // phase A has consumed the spins.  The periodic halo (row below, column to the right: tensor maps do not wrap) comes
 // through plain loads issued while the box is in flight.
-template <int MODEL, bool OBS>
-__global__ void __launch_bounds__(TILE_THREADS, SW_LABEL_MINB)
-k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, const __grid_constant__ CUtensorMap spin_map,
+// BATCH: blockIdx.x is a global tile of a batch (BatchView above); the lattice's Philox key then lives in registers
+// instead of the constant bank, which costs the fifth resident CTA.
+template <int MODEL, bool OBS, bool BATCH>
+__global__ void __launch_bounds__(TILE_THREADS, BATCH ? 4 : SW_LABEL_MINB)
+k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, const __grid_constant__ CUtensorMap spin_map,
              uint16_t *lab16, unsigned long long *parent, uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount,
-             int fuse, unsigned long long *stats, unsigned long long *obs)
+             int fuse, unsigned long long *stats, unsigned long long *obs, BatchView bv)
 {
     // OBS (q = 2 Potts only, "+ measurement" of PAPER.md:75): S5 fused into phase A.  With two states the
     // XOR of a spin word with its +x / +y neighbour word has byte 1 exactly on the unequal bonds, so three POPC per four
@@ -239,9 +249,22 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, const __
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t tiles_x = L / TW;
-    const uint32_t tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
+    const uint32_t lat = BATCH ? blockIdx.x / bv.tiles_per_lattice : 0u;          // lattice of the batch
+    const uint32_t ltile = BATCH ? blockIdx.x - lat * bv.tiles_per_lattice : blockIdx.x;
+    const uint32_t tx = ltile % tiles_x, ty = ltile / tiles_x;
     const uint32_t x0 = tx * TW, y0 = ty * TH;
     const uint32_t q2 = 2u * (uint32_t)md.q;
+    PhiloxKey key_lat;
+    if (BATCH) {
+        key_lat = bv.keys[lat];
+        md.thr_potts = bv.thr[lat];
+        md.table = bv.tables + (size_t)lat * (2 * 16) * (2 * 16);
+        spins += (size_t)lat * md.N;
+        lab16 += (size_t)lat * md.N;
+        hedge += (size_t)lat * tiles_x * (L / 32);
+        vedge += (size_t)lat * (L / TH) * (L / 32);
+    }
+    const PhiloxKey &key = BATCH ? key_lat : key_one;
     // per-phase clocks (lane 0 of every warp), only when the work counters are on: stats[8 + phase]
     long long ph_t = stats ? clock64() : 0;
 #define SW_PHASE(i)                                                                     \
@@ -258,7 +281,7 @@ k_tile_label(Model md, PhiloxKey key, uint32_t t, const uint8_t *spins, const __
     (void)o_neq; (void)o_one; (void)s_obs;
     if (tid == 0u) {                 // after griddepcontrol.wait: the spins of S^t are complete
         mbar_arrive_expect_tx(&s_bar, (uint32_t)TILE_SITES);
-        tma_load_2d(s_ew, &spin_map, x0, y0, &s_bar);
+        tma_load_2d(s_ew, &spin_map, x0, (BATCH ? lat * L : 0u) + y0, &s_bar);   // batch map: [B * L][L], lattices stacked
     }
     if (MODEL == 1) {
         for (uint32_t k = tid; k < q2 * q2; k += TILE_THREADS) s_table[k] = md.table[k];
@@ -774,30 +797,36 @@ __device__ __forceinline__ uint32_t groot_site_compress(unsigned long long *pare
 // bonds.  The two ends of an active tile-crossing bond lie in open clusters; their lab16 values (LOPEN | pos) come
 // from the compact edge arrays K1 wrote.
 constexpr int SEAM_THREADS = 256;
+// nlat lattices (1 unless a batch): positions of lattice b are b * ne .. (b + 1) * ne - 1, its tiles b * tiles .. .
 __global__ void __launch_bounds__(SEAM_THREADS)
 k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint16_t *edges, unsigned long long *parent,
-             unsigned long long *stats)
+             unsigned long long *stats, uint32_t nlat)
 {
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tiles_x = L / TW, tiles_y = L / TH;
     const uint32_t nh = tiles_x * L, ne = nh + tiles_y * L;
-    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
     pdl_prologue();
-    if (e >= ne) return;
+    if (e >= ne * nlat) return;
+    const uint32_t lat = e / ne;          // ne is a multiple of 32: uniform in a warp
+    e -= lat * ne;
+    hedge += (size_t)lat * tiles_x * (L / 32);
+    vedge += (size_t)lat * tiles_y * (L / 32);
+    const uint32_t tbase = lat * tiles_x * tiles_y;      // node keys carry GLOBAL node numbers: tiles stay global
     uint32_t bit, ta, tb, ia, ib;
     if (e < nh) {
         const uint32_t tx = e / L, y = e - tx * L;
         bit = (hedge[tx * (L / 32) + (y >> 5)] >> (y & 31u)) & 1u;
-        ta = (y / TH) * tiles_x + tx;
-        tb = (y / TH) * tiles_x + (tx + 1u == tiles_x ? 0u : tx + 1u);
+        ta = tbase + (y / TH) * tiles_x + tx;
+        tb = tbase + (y / TH) * tiles_x + (tx + 1u == tiles_x ? 0u : tx + 1u);
         ia = TH + y % TH;                     // right column of ta
         ib = y % TH;                          // left column of tb
     } else {
         const uint32_t f = e - nh;
         const uint32_t ty = f / L, x = f - ty * L;
         bit = (vedge[ty * (L / 32) + (x >> 5)] >> (x & 31u)) & 1u;
-        ta = ty * tiles_x + x / TW;
-        tb = (ty + 1u == tiles_y ? 0u : ty + 1u) * tiles_x + x / TW;
+        ta = tbase + ty * tiles_x + x / TW;
+        tb = tbase + (ty + 1u == tiles_y ? 0u : ty + 1u) * tiles_x + x / TW;
         ia = 2 * TH + TW + x % TW;            // bottom row of ta
         ib = 2 * TH + x % TW;                 // top row of tb
     }
@@ -814,10 +843,10 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
 }
 
 // K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).  in = S^t, out = S^{t+1}.
-template <int MODEL>
+template <int MODEL, bool BATCH>
 __global__ void __launch_bounds__(TILE_THREADS)
-k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *lab16, unsigned long long *parent, const uint32_t *ocount,
-            const uint8_t *in, uint8_t *out)
+k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsigned long long *parent, const uint32_t *ocount,
+            const uint8_t *in, uint8_t *out, BatchView bv)
 {
     constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
     __shared__ uint8_t s_dec[OCAP + NDEC];   // [pos] decision of the tile's open root pos; [DEC_BASE + d] = d
@@ -825,8 +854,18 @@ k_tile_flip(Model md, PhiloxKey key, uint32_t t, const uint16_t *lab16, unsigned
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tid = threadIdx.x;
     const uint32_t tiles_x = L / TW;
-    const uint32_t tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
+    const uint32_t lat = BATCH ? blockIdx.x / bv.tiles_per_lattice : 0u;
+    const uint32_t ltile = BATCH ? blockIdx.x - lat * bv.tiles_per_lattice : blockIdx.x;
+    const uint32_t tx = ltile % tiles_x, ty = ltile / tiles_x;
     const uint32_t x0 = tx * TW, y0 = ty * TH;
+    PhiloxKey key_lat;
+    if (BATCH) {
+        key_lat = bv.keys[lat];
+        lab16 += (size_t)lat * md.N;
+        in += (size_t)lat * md.N;
+        out += (size_t)lat * md.N;
+    }
+    const PhiloxKey &key = BATCH ? key_lat : key_one;
 
     pdl_prologue();
     // one decision per open root of the tile (S3; R5 CLUSTER stream), keyed on the site index of the root
@@ -903,9 +942,9 @@ __global__ void k_resolve_labels(Model md, const uint16_t *lab16, const unsigned
 // ---------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------
-// Tensor map of one [L][L] uint8 spin buffer with a TW x TH box (no swizzle, no interleave).  The driver's encoder is
-// reached through the runtime (no link against libcuda).
-static inline int make_spin_map(CUtensorMap *map, const uint8_t *base, int L)
+// Tensor map of `rows` x L uint8 spins (one lattice: rows = L; a batch: its lattices stacked, rows = B * L) with a
+// TW x TH box (no swizzle, no interleave).  The driver's encoder is reached through the runtime (no link against libcuda).
+static inline int make_spin_map(CUtensorMap *map, const uint8_t *base, int L, size_t rows)
 {
     typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -919,7 +958,7 @@ static inline int make_spin_map(CUtensorMap *map, const uint8_t *base, int L)
             return -1;
         encode = reinterpret_cast<encode_fn>(fn);
     }
-    const cuuint64_t dims[2] = { (cuuint64_t)L, (cuuint64_t)L };      // innermost first
+    const cuuint64_t dims[2] = { (cuuint64_t)L, (cuuint64_t)rows };   // innermost first
     const cuuint64_t strides[1] = { (cuuint64_t)L };                  // bytes between rows
     const cuuint32_t box[2] = { (cuuint32_t)TW, (cuuint32_t)TH };
     const cuuint32_t estr[2] = { 1u, 1u };
@@ -929,51 +968,82 @@ static inline int make_spin_map(CUtensorMap *map, const uint8_t *base, int L)
     return r == CUDA_SUCCESS ? 0 : -1;
 }
 
-static inline int tiled_init(TiledState &st, const Model &md, char *ws, const uint8_t *spins_a, const uint8_t *spins_b)
+// Workspace of nlat lattices (labels, seam masks, edge labels, open counts), carved from ws; the union-find nodes
+// (nlat * tiles * OCAP * 8 bytes) are the caller's.
+static inline size_t tiled_workspace_bytes_n(int L, size_t nlat)
+{
+    if (!tiled_supported(L)) return 0;
+    const size_t N = (size_t)L * L;
+    const size_t tiles = (size_t)(L / TW) * (L / TH);
+    return nlat * 2 * N + 1024 + nlat * (size_t)(L / TW) * (L / 32) * 4 + 1024 + nlat * (size_t)(L / TH) * (L / 32) * 4 + 1024 +
+           nlat * tiles * ECNT * 2 + 1024 + nlat * tiles * 4 + 1024;
+}
+
+static inline int tiled_init(TiledState &st, const Model &md, char *ws, const uint8_t *spins_a, const uint8_t *spins_b, size_t nlat = 1)
 {
     const size_t L = (size_t)md.L;
     st.L = md.L;
+    st.nlat = (uint32_t)nlat;
     st.map_base[0] = spins_a;
     st.map_base[1] = spins_b;
-    if (make_spin_map(&st.map[0], spins_a, md.L) != 0 || make_spin_map(&st.map[1], spins_b, md.L) != 0) return -1;
+    if (make_spin_map(&st.map[0], spins_a, md.L, nlat * L) != 0 || make_spin_map(&st.map[1], spins_b, md.L, nlat * L) != 0) return -1;
     size_t off = 0;
     st.lab16 = reinterpret_cast<uint16_t *>(ws);
-    off += (2 * L * L + 1023) / 1024 * 1024;
+    off += (nlat * 2 * L * L + 1023) / 1024 * 1024;
     st.hedge = reinterpret_cast<uint32_t *>(ws + off);
-    off += ((L / TW) * (L / 32) * 4 + 1023) / 1024 * 1024;
+    off += (nlat * (L / TW) * (L / 32) * 4 + 1023) / 1024 * 1024;
     st.vedge = reinterpret_cast<uint32_t *>(ws + off);
-    off += ((L / TH) * (L / 32) * 4 + 1023) / 1024 * 1024;
+    off += (nlat * (L / TH) * (L / 32) * 4 + 1023) / 1024 * 1024;
     const size_t tiles = (L / TW) * (L / TH);
     st.edges = reinterpret_cast<uint16_t *>(ws + off);
-    off += (tiles * ECNT * 2 + 1023) / 1024 * 1024;
+    off += (nlat * tiles * ECNT * 2 + 1023) / 1024 * 1024;
     st.ocount = reinterpret_cast<uint32_t *>(ws + off);
+    st.bv.tiles_per_lattice = (uint32_t)tiles;
     return 0;
 }
 
 constexpr int TILED_NUM_KERNELS = 3;
 static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k_seam_merge", "k_tile_flip" };
 
+// st.batch: the BATCH instantiations over st.nlat lattices (keys, thresholds and tables from st.bv; `key` and the
+// thresholds inside `md` are then unused).
 static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
                                       unsigned long long *parent, int fuse, cudaStream_t stream, unsigned long long *stats,
                                       unsigned long long *obs = nullptr)
 {
-    const uint32_t tiles = ((uint32_t)md.L / TW) * ((uint32_t)md.L / TH);
+    const uint32_t tiles = ((uint32_t)md.L / TW) * ((uint32_t)md.L / TH) * st.nlat;
     if (g_pdl_dynamic_smem) {      // occupancy experiments only
-        cudaFuncSetAttribute(k_tile_label<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
-        cudaFuncSetAttribute(k_tile_label<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
+        cudaFuncSetAttribute(k_tile_label<0, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
+        cudaFuncSetAttribute(k_tile_label<1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g_pdl_dynamic_smem);
     }
     const int which = in == st.map_base[0] ? 0 : in == st.map_base[1] ? 1 : -1;
     if (which < 0) return cudaErrorInvalidValue;     // a spin buffer without a tensor map
     const CUtensorMap &tm = st.map[which];
     unsigned long long *const none = nullptr;
+    if (st.batch) {
+        if (md.model == 0)
+            return launch_pdl(k_tile_label<0, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+                              st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+        return launch_pdl(k_tile_label<1, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+    }
     if (md.model == 0 && md.q == 2 && obs)
-        return launch_pdl(k_tile_label<0, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge, st.vedge,
-                          st.edges, st.ocount, fuse, stats, obs);
+        return launch_pdl(k_tile_label<0, true, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+                          st.vedge, st.edges, st.ocount, fuse, stats, obs, st.bv);
     if (md.model == 0)
-        return launch_pdl(k_tile_label<0, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge, st.vedge,
-                          st.edges, st.ocount, fuse, stats, none);
-    return launch_pdl(k_tile_label<1, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge, st.vedge,
-                      st.edges, st.ocount, fuse, stats, none);
+        return launch_pdl(k_tile_label<0, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+    return launch_pdl(k_tile_label<1, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+                      st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+}
+
+static inline cudaError_t tiled_launch_merge(TiledState &st, const Model &md, unsigned long long *parent, cudaStream_t stream,
+                                             unsigned long long *stats)
+{
+    const uint32_t L = (uint32_t)md.L;
+    const uint32_t ne = ((L / TW) * L + (L / TH) * L) * st.nlat;
+    return launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent,
+                      stats, st.nlat);
 }
 
 // One sweep: in = S^t (left untouched), out = S^{t+1}.  ev (optional): ev[0] is recorded before the first kernel,
@@ -986,19 +1056,20 @@ static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &
                               uint64_t *launches, cudaEvent_t *ev, unsigned long long *obs = nullptr)
 {
     const uint32_t L = (uint32_t)md.L;
-    const uint32_t tiles = (L / TW) * (L / TH);
-    const uint32_t ne = (L / TW) * L + (L / TH) * L;
+    const uint32_t tiles = (L / TW) * (L / TH) * st.nlat;
     if (ev) cudaEventRecord(ev[0], stream);
     cudaError_t e = tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats, obs);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[1], stream);
-    e = launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent, stats);
+    e = tiled_launch_merge(st, md, parent, stream, stats);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[2], stream);
-    if (md.model == 0)
-        e = launch_pdl(k_tile_flip<0>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out);
+    if (st.batch)
+        e = md.model == 0 ? launch_pdl(k_tile_flip<0, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv)
+                          : launch_pdl(k_tile_flip<1, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv);
     else
-        e = launch_pdl(k_tile_flip<1>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out);
+        e = md.model == 0 ? launch_pdl(k_tile_flip<0, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv)
+                          : launch_pdl(k_tile_flip<1, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[3], stream);
     *launches += 3;
@@ -1010,11 +1081,8 @@ static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &
 static inline int tiled_relabel(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
                                 unsigned long long *parent, cudaStream_t stream, uint64_t *launches)
 {
-    const uint32_t L = (uint32_t)md.L;
-    const uint32_t ne = (L / TW) * L + (L / TH) * L;
     if (tiled_launch_label(st, md, key, t, in, parent, 0, stream, nullptr) != cudaSuccess) return -1;
-    if (launch_pdl(k_seam_merge, (ne + SEAM_THREADS - 1) / SEAM_THREADS, SEAM_THREADS, stream, md, st.hedge, st.vedge, st.edges, parent,
-                   (unsigned long long *)nullptr) != cudaSuccess) return -1;
+    if (tiled_launch_merge(st, md, parent, stream, nullptr) != cudaSuccess) return -1;
     *launches += 2;
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
 }

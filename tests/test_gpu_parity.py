@@ -210,11 +210,13 @@ def test_small_backend(sw, oracle, L, q, model, T):
         _assert_same(lat.get_labels(), olab, "labels of the last sweep")
 
 
-@pytest.mark.parametrize("L,q,model", [(64, 2, POTTS), (32, 3, POTTS), (48, 6, CLOCK), (128, 2, POTTS), (7, 4, CLOCK)])
+@pytest.mark.parametrize("L,q,model", [(64, 2, POTTS), (32, 3, POTTS), (48, 6, CLOCK), (128, 2, POTTS), (7, 4, CLOCK),
+                                       (256, 2, POTTS), (384, 3, POTTS), (256, 6, CLOCK)])
 def test_batch_every_lattice_equals_its_own_run(sw, oracle, L, q, model):
     """A batch of lattices with different temperatures and seeds: lattice b equals the single-lattice oracle run with
-    (T[b], seed[b]) after every call, and its histograms equal the oracle's."""
-    B = 11
+    (T[b], seed[b]) after every call, and its histograms equal the oracle's.  L <= 128: one CTA per lattice; L = 256, 384:
+    the tiles of all lattices in one grid per kernel."""
+    B = 11 if L <= 128 else 5
     base = tc(q) if model == POTTS else 0.9
     T = [base * (0.6 + 0.08 * b) for b in range(B)]
     seed = [0x5EED0200 + 7919 * b + (b << 40) for b in range(B)]
