@@ -44,7 +44,11 @@ enum {
     SW_ALGO_AUTO = 0,    /* one CTA when L <= 64, else tiled when L allows it, else generic */
     SW_ALGO_GENERIC = 1, /* whole-lattice union-find in global memory; any L >= 2 */
     SW_ALGO_TILED = 2,   /* tile-local union-find in shared memory + boundary merge; needs L % 128 == 0 */
-    SW_ALGO_SMALL = 3    /* one CTA owns the lattice in shared memory and runs all n sweeps of a call in one launch; L <= 128 */
+    SW_ALGO_SMALL = 3,   /* one CTA owns the lattice in shared memory and runs all n sweeps of a call in one launch; L <= 128 */
+    /* The paper's own labellers, kept as A/B references: whole-lattice label equivalence iterated from
+     * the host until a scan changes nothing; any L >= 2.  sw_stats reports their iteration counts. */
+    SW_ALGO_HAWICK = 4,  /* Hawick et al.: label + R arrays, scan (atomicMin) / analysis / labeling kernels */
+    SW_ALGO_KALENTEV = 5 /* Kalentev et al.: one array, scan / analysis kernels, no atomics */
 };
 
 /* Limits of the GPU path: 2 <= L <= 16384 (site index must leave 4 spare bits in an int32 label),
@@ -137,7 +141,8 @@ int sw_get_algorithm(sw_ctx *ctx); /* the back-end actually in use (never SW_ALG
 /* Labeling work counters accumulated since creation (the analogue of the paper's iteration counts,
  * PAPER.md:75), HOST output of SW_NUM_STATS doubles: out[0] = sweeps counted, out[1] = cross-tile merge attempts,
  * out[2] = tile-local nodes (horizontal runs), out[3] = tile-local union edges, out[4] = pointer hops of the
- * tile-local resolve pass, out[5..7] reserved (0), out[8..15] = SM clock cycles the warps of the tile-labeling
+ * tile-local resolve pass, out[5] = scan passes of the paper's labellers (SW_ALGO_HAWICK / SW_ALGO_KALENTEV, always
+ * counted) and out[6] = the sweeps they served (out[5] / out[6] is the iteration count PAPER.md:75 quotes), out[7] reserved (0), out[8..15] = SM clock cycles the warps of the tile-labeling
  * kernel spent in each of its phases (bonds, setup, run scan, unions, open marking, resolve, output, root decisions;
  * summed over warps).  Counters are only collected after sw_enable_stats(ctx, 1) (they cost atomics and clock reads). */
 #define SW_NUM_STATS 16

@@ -23,7 +23,7 @@ LIB_PATH = Path(os.environ["SW_LIB"]) if os.environ.get("SW_LIB") else _PKG / "l
 
 SW_POTTS, SW_CLOCK = 0, 1
 SW_OK, SW_ERR_ARG, SW_ERR_CUDA, SW_ERR_NOMEM, SW_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
-SW_ALGO_AUTO, SW_ALGO_GENERIC, SW_ALGO_TILED, SW_ALGO_SMALL = 0, 1, 2, 3
+SW_ALGO_AUTO, SW_ALGO_GENERIC, SW_ALGO_TILED, SW_ALGO_SMALL, SW_ALGO_HAWICK, SW_ALGO_KALENTEV = 0, 1, 2, 3, 4, 5
 
 # name -> (restype, argtypes): every symbol include/sw.h declares
 _vp, _i, _u64, _d, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_uint64, ctypes.c_double, ctypes.c_size_t

@@ -15,6 +15,7 @@
 
 #include "sw.h"
 #include "sw_generic.cuh"
+#include "sw_paper_ccl.cuh"
 #include "sw_philox.cuh"
 #include "sw_small.cuh"
 #include "sw_tile.cuh"
@@ -52,7 +53,7 @@ bool args_ok(int L, int q, int model)
 }
 
 struct Carve {
-    size_t spins, spins2, labels, bonds, table, obs, flag, stats, ring, small, tiled, total;
+    size_t spins, spins2, labels, labels2, bonds, table, obs, flag, stats, ring, small, tiled, total;
 };
 
 Carve carve(int L, int q)
@@ -64,6 +65,7 @@ Carve carve(int L, int q)
     c.spins = off;  off += align_up(N);
     c.spins2 = off; off += align_up(N);
     c.labels = off; off += align_up(4 * N);
+    c.labels2 = off; off += align_up(4 * N);     // R of the Hawick labeller (SW_ALGO_HAWICK)
     c.bonds = off;  off += align_up(N);
     c.table = off;  off += align_up(4 * (size_t)(2 * SW_MAX_Q) * (2 * SW_MAX_Q));
     c.obs = off;    off += align_up(8 * OBS_WORDS);
@@ -89,7 +91,7 @@ struct sw_ctx {
     char *ws = nullptr;
     Carve cv{};
     uint8_t *spins = nullptr, *spins_alt = nullptr, *bonds = nullptr;  // spins = S^t; spins_alt = the other buffer of the tiled ping-pong
-    int32_t *labels = nullptr;
+    int32_t *labels = nullptr, *labels2 = nullptr;
     uint32_t *table = nullptr;
     unsigned long long *obs = nullptr, *stats = nullptr, *ring = nullptr;
     int *flag = nullptr;
@@ -102,6 +104,7 @@ struct sw_ctx {
     bool have_labels = false, stats_on = false;
     int last_algo = 0;
     uint64_t launches = 0, stat_sweeps = 0;
+    uint64_t ccl_iterations = 0, ccl_sweeps = 0;   // SW_ALGO_HAWICK / SW_ALGO_KALENTEV: scan passes and the sweeps they served
     sw::TiledState tiled{};
     unsigned long long *rec_host = nullptr;   // pinned copy of the record ring (sw_sweep_record)
 };
@@ -150,6 +153,26 @@ void build_thresholds(sw_ctx *c)
 inline unsigned blocks_for(size_t n, unsigned bs) { return (unsigned)((n + bs - 1) / bs); }
 
 const char *const GENERIC_KERNELS[] = { "k_bonds", "k_label_init", "k_union", "k_flatten", "k_flip" };
+
+// One sweep with one of the paper's own labellers: bonds -> iterated label equivalence -> flip.
+int paper_sweep(sw_ctx *c, uint32_t t, cudaEvent_t *ev)
+{
+    const unsigned bs = 256;
+    const uint32_t N = c->md.N;
+    if (ev) cudaEventRecord(ev[0], c->stream);
+    sw::k_bonds<<<blocks_for((N + 1) / 2, bs), bs, 0, c->stream>>>(c->md, c->key, t, c->spins, c->bonds);
+    if (ev) cudaEventRecord(ev[1], c->stream);
+    const int it = sw::paper_ccl_label(c->algo == SW_ALGO_KALENTEV, c->md, c->bonds, c->labels, c->labels2, c->flag, c->stream, &c->launches);
+    if (it < 0) return fail(SW_ERR_CUDA, "paper labeller failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->ccl_iterations += (uint64_t)it;
+    c->ccl_sweeps += 1;
+    if (ev) cudaEventRecord(ev[2], c->stream);
+    sw::k_flip<<<blocks_for(N, bs), bs, 0, c->stream>>>(c->md, c->key, t, c->labels, c->spins);
+    if (ev) cudaEventRecord(ev[3], c->stream);
+    c->launches += 2;
+    CU_TRY(cudaPeekAtLastError());
+    return SW_OK;
+}
 
 // SW_ALGO_AUTO: one CTA for L <= 64 (measured: 7 us per sweep at L = 32 and 26 us at L = 64 against 22 and 28 us of
 // the five generic launches; at L = 128 the single CTA is the slower one), tiles when L allows them, else generic
@@ -205,6 +228,8 @@ int one_sweep(sw_ctx *c, cudaEvent_t *ev = nullptr, unsigned long long *obs_row 
         std::swap(c->spins, c->spins_alt);   // spins_alt now holds S^t, the input of this sweep
     } else if (c->algo == SW_ALGO_SMALL) {
         rc = small_sweeps(c, 1, ev);
+    } else if (c->algo == SW_ALGO_HAWICK || c->algo == SW_ALGO_KALENTEV) {
+        rc = paper_sweep(c, t, ev);
     } else {
         rc = generic_sweep(c, t, ev);
     }
@@ -300,6 +325,7 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
     c->spins = (uint8_t *)(c->ws + c->cv.spins);
     c->spins_alt = (uint8_t *)(c->ws + c->cv.spins2);
     c->labels = (int32_t *)(c->ws + c->cv.labels);
+    c->labels2 = (int32_t *)(c->ws + c->cv.labels2);
     c->bonds = (uint8_t *)(c->ws + c->cv.bonds);
     c->table = (uint32_t *)(c->ws + c->cv.table);
     c->obs = (unsigned long long *)(c->ws + c->cv.obs);
@@ -599,7 +625,7 @@ int sw_set_algorithm(sw_ctx *c, int algo)
         return fail(SW_ERR_UNSUPPORTED, "sw_set_algorithm: the tiled back-end needs L %% %d == 0 (L = %d)", sw::TW, c->L);
     if (algo == SW_ALGO_SMALL && !sw::small_supported(c->L))
         return fail(SW_ERR_UNSUPPORTED, "sw_set_algorithm: the one-CTA back-end needs L <= %d (L = %d)", sw::SMALL_MAX_L, c->L);
-    if (algo != SW_ALGO_GENERIC && algo != SW_ALGO_TILED && algo != SW_ALGO_SMALL)
+    if (algo != SW_ALGO_GENERIC && algo != SW_ALGO_TILED && algo != SW_ALGO_SMALL && algo != SW_ALGO_HAWICK && algo != SW_ALGO_KALENTEV)
         return fail(SW_ERR_ARG, "sw_set_algorithm: unknown back-end %d", algo);
     c->algo = algo;
     return SW_OK;
@@ -623,6 +649,8 @@ int sw_stats(sw_ctx *c, double *out4)
     CU_TRY(cudaStreamSynchronize(c->stream));
     for (int k = 0; k < SW_NUM_STATS; ++k) out4[k] = (double)h[k];
     out4[0] = (double)c->stat_sweeps;
+    out4[5] = (double)c->ccl_iterations;
+    out4[6] = (double)c->ccl_sweeps;
     return SW_OK;
 }
 
@@ -631,7 +659,8 @@ int sw_sweep_profile(sw_ctx *c, int n, double *ms_out, int *n_kernels)
     if (!c || n < 0 || !ms_out || !n_kernels) return fail(SW_ERR_ARG, "sw_sweep_profile: bad arguments");
     DeviceGuard guard(c);
     if (c->t + (uint64_t)n > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_profile: sweep index would exceed 2^32-1");
-    const int nk = (c->algo == SW_ALGO_TILED) ? sw::TILED_NUM_KERNELS : (c->algo == SW_ALGO_SMALL) ? 1 : 5;
+    const int nk = (c->algo == SW_ALGO_TILED) ? sw::TILED_NUM_KERNELS : (c->algo == SW_ALGO_SMALL) ? 1 :
+                   (c->algo == SW_ALGO_HAWICK || c->algo == SW_ALGO_KALENTEV) ? 3 : 5;
     cudaEvent_t ev[SW_MAX_KERNELS + 1];
     for (int k = 0; k <= nk; ++k) CU_TRY(cudaEventCreate(&ev[k]));
     for (int k = 0; k < SW_MAX_KERNELS; ++k) ms_out[k] = 0.0;
@@ -656,6 +685,10 @@ const char *sw_kernel_name(sw_ctx *c, int k)
     if (!c || k < 0) return nullptr;
     if (c->algo == SW_ALGO_TILED) return k < sw::TILED_NUM_KERNELS ? sw::TILED_KERNELS[k] : nullptr;
     if (c->algo == SW_ALGO_SMALL) return k == 0 ? "k_small_sweeps" : nullptr;
+    if (c->algo == SW_ALGO_HAWICK || c->algo == SW_ALGO_KALENTEV) {
+        static const char *const names[3] = { "k_bonds", "label equivalence (all iterations)", "k_flip" };
+        return k < 3 ? names[k] : nullptr;
+    }
     return k < 5 ? GENERIC_KERNELS[k] : nullptr;
 }
 

@@ -15,7 +15,7 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 POTTS, CLOCK = 0, 1
-GENERIC, TILED, SMALL = 1, 2, 3
+GENERIC, TILED, SMALL, HAWICK, KALENTEV = 1, 2, 3, 4, 5
 
 
 @pytest.fixture(scope="module")
@@ -247,6 +247,39 @@ def test_batch_every_lattice_equals_its_own_run(sw, oracle, L, q, model):
         got = bt.get_spins()
         for b in range(B):
             _assert_same(got[b], oracle.run(L, q, model, T[b], seed[b], 40, 2, s0[b]), f"lattice {b} after the hand-off")
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4: the paper's own labellers as A/B back-ends, with their iteration counts
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("algo", [HAWICK, KALENTEV])
+@pytest.mark.parametrize("L,q,model,T", [(2, 2, POTTS, tc(2)), (5, 3, POTTS, tc(3)), (31, 6, CLOCK, 0.9), (64, 2, POTTS, tc(2)),
+                                          (128, 2, POTTS, 0.8 * tc(2)), (256, 2, POTTS, tc(2)), (100, 4, POTTS, 1e6), (48, 2, POTTS, 0.02)])
+def test_paper_labellers_reach_the_oracle_labels(sw, oracle, algo, L, q, model, T):
+    """Converged label equivalence = smallest site index of the cluster: labels, spins and histograms equal
+    the oracle's after every sweep."""
+    run_and_compare(sw, oracle, L, q, model, T, seed=0x5EED0400 + L, algo=algo, n=3)
+
+
+@pytest.mark.parametrize("algo", [HAWICK, KALENTEV])
+def test_paper_labellers_iteration_counts(sw, algo):
+    """PAPER.md:75 quotes 6.6 / 7.1 iterations per sweep at Tc for L = 256 / 512 (q = 2).  The count depends on details the
+    paper does not give (scan order, what counts as an iteration), so only the scale and the slow growth with L are
+    checked: a handful of whole-lattice passes, more at L = 512 than at L = 256, one pass when nothing is bonded."""
+    its = {}
+    for L in (256, 512):
+        with sw.Lattice(L, 2, POTTS, tc(2), 0x5EED0401, algo=algo) as lat:
+            lat.sweep(60)                               # equilibrate: the cluster structure sets the count
+            st0 = lat.stats()
+            lat.sweep(40)
+            st1 = lat.stats()
+            its[L] = (st1[5] - st0[5]) / (st1[6] - st0[6])
+            print(f"algo {algo} L={L}: {its[L]:.2f} iterations per sweep at Tc (paper: {6.6 if L == 256 else 7.1})")
+    assert 3.0 <= its[256] <= 20.0 and 3.0 <= its[512] <= 20.0 and its[512] >= its[256] - 0.5
+    with sw.Lattice(64, 2, POTTS, 1e6, 1, algo=algo) as lat:    # p -> 0: no bond, the first scan changes nothing
+        lat.sweep(3)
+        st = lat.stats()
+        assert st[5] == 3 and st[6] == 3
 
 
 # ------------------------------------------------------------------------------------------------
