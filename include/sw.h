@@ -179,6 +179,34 @@ int sw_batch_set_spins(sw_batch *batch, const uint8_t *host_in, uint64_t sweep_i
 int sw_batch_observables(sw_batch *batch, int64_t *bond_hist, int64_t *state_hist);
 uint64_t sw_batch_sweep_index(sw_batch *batch);
 
+/* NEXT-3 of the scope table: ONE lattice sharded over `nranks` ranks by row stripes (the paper's own outlook, PAPER.md:193;
+ * scheme: SURVEY.md 8(e)).  Rank r owns rows [r L / nranks, (r + 1) L / nranks); needs L % nranks == 0 and L % 4 == 0.
+ * One sweep is four calls per rank, with two exchanges between them that are the caller's (torch.distributed in
+ * paper_1202_0635_b200/stripes.py: NCCL between GPUs, gloo in the CPU test of the host logic):
+ *   sw_stripe_first_row    HOST out, L bytes: my first row of spins -- the halo of the previous rank (periodic)
+ *   sw_stripe_label        HOST in, L bytes: the first row of the NEXT rank.  Bonds of my sites (Philox keyed on global
+ *                          site indices: exactly the bonds of the single-GPU run) and labels inside my stripe
+ *   sw_stripe_export_seam  HOST out, L entries each: global index of the local root of every site of my first row, of
+ *                          my last row, and whether the +y bond of my last row is active.  All ranks gather these.
+ *   sw_seam_solve          pure host code (no device needed), identical on every rank: first / last / seam are the
+ *                          gathered [nranks][L] arrays; union-find by minimum index over the seam pairs; out: the local
+ *                          roots whose canonical root differs from themselves, from[k] -> to[k], k < *n_map <= 2 nranks L
+ *   sw_stripe_finish       HOST in: that map.  Decisions keyed on the global canonical root, spin update; sweep index + 1
+ * The spins after every sweep equal those of the single-GPU run bit for bit.  sw_stripe_get_labels: canonical roots of
+ * the last finished sweep (rows * L int32).  NULL / SW_ERR_* as everywhere. */
+typedef struct sw_stripe sw_stripe;
+sw_stripe *sw_stripe_create(int L, int q, int model, double T, uint64_t seed, int rank, int nranks);
+void sw_stripe_destroy(sw_stripe *stripe);
+int sw_stripe_first_row(sw_stripe *stripe, uint8_t *host_out);
+int sw_stripe_label(sw_stripe *stripe, const uint8_t *halo_row_host);
+int sw_stripe_export_seam(sw_stripe *stripe, int32_t *first_row_labels, int32_t *last_row_labels, uint8_t *seam_bonds);
+int sw_seam_solve(int nranks, int L, const int32_t *first, const int32_t *last, const uint8_t *seam, int32_t *from, int32_t *to, int *n_map);
+int sw_stripe_finish(sw_stripe *stripe, int n_map, const int32_t *from, const int32_t *to);
+int sw_stripe_get_spins(sw_stripe *stripe, uint8_t *host_out);
+int sw_stripe_get_labels(sw_stripe *stripe, int32_t *host_out);
+int sw_stripe_set_spins(sw_stripe *stripe, const uint8_t *host_in, uint64_t sweep_index);
+uint64_t sw_stripe_sweep_index(sw_stripe *stripe);
+
 /* Instruction-issue probes (measurement infrastructure for the "alu" roofline of DESIGN.md section 6; the sweep never
  * uses them).  Probe `probe` (0 .. until sw_microbench_name returns NULL) runs `warps_per_smsp` (1..16) warps on every
  * SM sub-partition of the current device, each executing `iters` loop iterations of 8 independent dependency chains of

@@ -66,6 +66,17 @@ SYMBOLS = {
     "sw_batch_set_spins": (_i, [_vp, _vp, _u64]),
     "sw_batch_observables": (_i, [_vp, _vp, _vp]),
     "sw_batch_sweep_index": (_u64, [_vp]),
+    "sw_stripe_create": (_vp, [_i, _i, _i, _d, _u64, _i, _i]),
+    "sw_stripe_destroy": (None, [_vp]),
+    "sw_stripe_first_row": (_i, [_vp, _vp]),
+    "sw_stripe_label": (_i, [_vp, _vp]),
+    "sw_stripe_export_seam": (_i, [_vp, _vp, _vp, _vp]),
+    "sw_seam_solve": (_i, [_i, _i, _vp, _vp, _vp, _vp, _vp, ctypes.POINTER(_i)]),
+    "sw_stripe_finish": (_i, [_vp, _i, _vp, _vp]),
+    "sw_stripe_get_spins": (_i, [_vp, _vp]),
+    "sw_stripe_get_labels": (_i, [_vp, _vp]),
+    "sw_stripe_set_spins": (_i, [_vp, _vp, _u64]),
+    "sw_stripe_sweep_index": (_u64, [_vp]),
     "sw_microbench": (_i, [_i, _i, _i, _vp]),
     "sw_microbench_name": (ctypes.c_char_p, [_i]),
     "sw_selftest": (_i, []),

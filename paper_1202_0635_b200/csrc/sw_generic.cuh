@@ -67,7 +67,7 @@ __device__ __forceinline__ uint32_t clock_c4(uint32_t w, uint32_t m, uint32_t q2
     return t - (ge >> 7) * q2;
 }
 
-__global__ void k_init_spins(Model md, PhiloxKey key, uint8_t *__restrict__ spins)
+static __global__ void k_init_spins(Model md, PhiloxKey key, uint8_t *__restrict__ spins)
 {
     const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;  // group of 4 sites
     const uint32_t base = g * 4u;
@@ -80,7 +80,7 @@ __global__ void k_init_spins(Model md, PhiloxKey key, uint8_t *__restrict__ spin
 }
 
 // One thread per pair of sites (2p, 2p+1): one Philox call gives the four words of the pair.
-__global__ void k_bonds(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ spins,
+static __global__ void k_bonds(Model md, PhiloxKey key, uint32_t t, const uint8_t *__restrict__ spins,
                         uint8_t *__restrict__ bonds)
 {
     const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
@@ -111,7 +111,7 @@ __global__ void k_bonds(Model md, PhiloxKey key, uint32_t t, const uint8_t *__re
     }
 }
 
-__global__ void k_label_init(uint32_t N, int32_t *__restrict__ labels)
+static __global__ void k_label_init(uint32_t N, int32_t *__restrict__ labels)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < N) labels[i] = (int32_t)i;
@@ -157,7 +157,7 @@ __device__ __forceinline__ void uf_union(int32_t *lab, int32_t a, int32_t b)
     }
 }
 
-__global__ void k_union(Model md, const uint8_t *__restrict__ bonds, int32_t *labels)
+static __global__ void k_union(Model md, const uint8_t *__restrict__ bonds, int32_t *labels)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= md.N) return;
@@ -174,13 +174,13 @@ __global__ void k_union(Model md, const uint8_t *__restrict__ bonds, int32_t *la
     }
 }
 
-__global__ void k_flatten(uint32_t N, int32_t *labels)
+static __global__ void k_flatten(uint32_t N, int32_t *labels)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < N) labels[i] = uf_find(labels, (int32_t)i);
 }
 
-__global__ void k_flip(Model md, PhiloxKey key, uint32_t t, const int32_t *__restrict__ labels,
+static __global__ void k_flip(Model md, PhiloxKey key, uint32_t t, const int32_t *__restrict__ labels,
                        uint8_t *__restrict__ spins)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -377,7 +377,7 @@ __global__ void __launch_bounds__(HIST_THREADS) k_correlation(Model md, const ui
 }
 
 // Validation of a configuration handed in by sw_set_spins: flag[0] = 1 if any value >= q.
-__global__ void k_check_spins(uint32_t N, uint32_t q, const uint8_t *__restrict__ spins, int *flag)
+static __global__ void k_check_spins(uint32_t N, uint32_t q, const uint8_t *__restrict__ spins, int *flag)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < N && spins[i] >= q) *flag = 1;
