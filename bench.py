@@ -133,6 +133,50 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def load_capture(kernel: str, workload: str):
+    """Per-launch counts of `kernel` from the committed ncu capture (profiles/traffic.json, written by
+    `python -m paper_1202_0635_b200.ncu_summary --record`), or None if there is none for this workload or if the kernel
+    sources changed since it was taken (the hash of csrc/ is stored with it)."""
+    tr = ROOT / "profiles" / "traffic.json"
+    if not tr.exists():
+        return None
+    try:
+        from paper_1202_0635_b200.ncu_summary import csrc_sha256
+        cap = json.loads(tr.read_text()).get(f"{kernel}@{workload}")
+        if cap is None or cap.get("csrc_sha256") != csrc_sha256():
+            return None
+        return cap
+    except Exception:
+        return None
+
+
+def run_batch(args, w, seed):
+    """NEXT-2: B lattices of the workload's (L, q, model, T), own seeds, advanced together (sw_create_batch).  One JSON line."""
+    import torch
+    from paper_1202_0635_b200 import binding as sw
+    B, N = args.batch, w.L * w.L
+    bt = sw.Batch(w.L, w.q, w.model, [w.T] * B, [seed + 7919 * b for b in range(B)])
+    bt.sweep(args.equil)
+    sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
+    sampler.start()
+    for _ in range(3):
+        bt.sweep(max(1, args.warmup // 3))
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    bt.sweep(args.steps)                              # synchronous at return
+    dt = time.perf_counter() - t0
+    clocks = sampler.stop()
+    print(json.dumps({
+        "metric": "ns per spin flip (full SW sweep), batch of lattices", "value": dt * 1e9 / (args.steps * B * N), "unit": UNIT, "n_gpus": 1,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u8 spins / int32 labels / u32 Philox", "data": "synthetic",
+        "config": {"workload": f"batch of {B} x {w.name}", "B": B, "L": w.L, "q": w.q, "model": "potts" if w.model == 0 else "clock", "T": w.T,
+                   "equil_sweeps": args.equil, "timing": "host clock around one synchronous sw_batch_sweep(steps)",
+                   "backend": "tiles of all lattices in one grid" if w.L % 128 == 0 else "one CTA per lattice"},
+        "clocks": clocks}), flush=True)
+    bt.close()
+
+
 def run_microbench(args):
     """Issue-rate probes (sw_microbench): warp-instructions per SM cycle per sub-partition, per opcode and mix.
     Prints one JSON line per probe and a markdown table (the table is what profiles/ keeps)."""
@@ -178,6 +222,9 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default=None, help="a key of workloads.CONFIGS (default: the headline config)")
     ap.add_argument("--equil", type=int, default=300, help="untimed sweeps from the random start before warm-up")
+    ap.add_argument("--algo", default="auto", choices=["auto", "generic", "tiled", "small", "hawick", "kalentev"],
+                    help="labeling back-end (sw_set_algorithm); hawick / kalentev are the paper's own labellers (A/B reference)")
+    ap.add_argument("--batch", type=int, default=0, help="B > 0: time a batch of B lattices of the workload's (L, q, model, T) (sw_create_batch)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
@@ -209,7 +256,11 @@ def main():
     L, q, N = w.L, w.q, w.L * w.L
     from paper_1202_0635_b200 import replicas
     seed = replicas.replica_seed(w.seed, rank)       # replicas only: every rank its own lattice
-    lat = sw.Lattice(L, q, w.model, w.T, seed)
+    if args.batch > 0:
+        run_batch(args, w, seed)
+        return
+    ALGOS = {"auto": 0, "generic": 1, "tiled": 2, "small": 3, "hawick": 4, "kalentev": 5}
+    lat = sw.Lattice(L, q, w.model, w.T, seed, algo=ALGOS[args.algo])
     stream = torch.cuda.current_stream()
     l2_flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
@@ -260,6 +311,8 @@ def main():
     barrier()
     meas_ms = m0.elapsed_time(m1)
     clocks = sampler.stop()
+    st = lat.stats()
+    iters_per_sweep = float(st[5] / st[6]) if st[6] > 0 else None     # the paper's labellers only (6.6-8.6 at Tc)
 
     # ---- per-kernel device time (events between kernels), L2 flushed before each sweep ----------------------
     prof = {}
@@ -272,23 +325,29 @@ def main():
     dom = max(prof, key=prof.get)
     peak, peak_src = peaks()
     dom_bytes = B_ALG_KERNEL.get(dom, 5.0) * N
-    achieved = dom_bytes / (prof[dom] * 1e-3) / 1e9
-    traffic, issue = None, None
-    tr = ROOT / "profiles" / "traffic.json"
-    if tr.exists() and w.name == HEADLINE:
-        try:
-            tj = json.loads(tr.read_text())
-            traffic = tj.get(dom)
-            winst, dcyc = tj.get(dom + "_warp_instructions"), tj.get(dom + "_dispatch_cycles")
-            if winst and dcyc:
-                # the bound DESIGN.md sections 6 and 11 derive: math-dispatch cycles, 148 SMs x 4 schedulers x SM clock
-                # (an ALU-pipe or IMAD.WIDE warp instruction takes two dispatch cycles, a 32-bit IMAD one)
-                ipeak = 148 * 4 * (clocks["sm_mhz"] or 1965.0) * 1e6
-                issue = {"bound": "alu", "achieved": dcyc / (prof[dom] * 1e-3), "peak": ipeak, "unit": "dispatch-cycles/s",
-                         "frac": dcyc / (prof[dom] * 1e-3) / ipeak, "warp_instructions_per_launch": winst,
-                         "source": "executed-opcode histogram of the committed ncu capture (profiles/r1_final.md) / live kernel time"}
-        except Exception:
-            traffic = None
+    t_dom = prof[dom] * 1e-3                                          # seconds per launch of the dominant kernel
+    hbm_nominal = {"bytes_per_launch": dom_bytes, "achieved": dom_bytes / t_dom / 1e9, "peak": peak, "unit": "GB/s",
+                   "frac": dom_bytes / t_dom / 1e9 / peak, "peak_source": peak_src,
+                   "note": "SURVEY 8(d) accounting (int32 labels: 1 + 4 B/site); this kernel moves 1 + 2 B/site"}
+    roofline = dict(hbm_nominal, bound="hbm", kernel=dom, traffic=None, ms_per_launch=prof[dom])
+    cap = load_capture(dom, w.name)
+    if cap is not None:
+        # The dominant kernel is bound by the integer ALU pipe, not by HBM: achieved = ALU-pipe busy
+        # cycles per launch (2 per ALU-class warp-instruction and 2 per IMAD.WIDE, rates measured by `bench.py --microbench`,
+        # counts from the committed ncu capture of this very source) / live kernel time; peak = sub-partitions x SM clock.
+        sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+        clk_hz = (clocks["sm_mhz"] or 1965.0) * 1e6
+        apeak = sms * 4 * clk_hz
+        roofline = {"bound": "alu", "kernel": dom, "achieved": cap["alu_pipe_cycles"] / t_dom, "peak": apeak, "unit": "ALU-pipe busy cycles/s",
+                    "frac": cap["alu_pipe_cycles"] / t_dom / apeak, "traffic": cap["dram_bytes"], "ms_per_launch": prof[dom],
+                    "peak_source": f"{sms} SMs x 4 sub-partitions x {clk_hz / 1e6:.0f} MHz (one ALU-pipe cycle per sub-partition and clock)",
+                    "warp_instructions_per_launch": cap["warp_instructions"],
+                    "other_pipes": {k: cap[k + "_pipe_cycles"] / t_dom / apeak for k in ("fma", "xu", "lsu")},
+                    "issue_slots": cap["warp_instructions"] / t_dom / apeak,
+                    "model": "profiles/r2_microbench.md (measured issue rates) applied to the opcode histogram of profiles/" + cap["report"],
+                    "hbm_nominal": hbm_nominal,
+                    "hbm_measured": {"bytes_per_launch": cap["dram_bytes"], "achieved": cap["dram_bytes"] / t_dom / 1e9, "peak": peak,
+                                     "unit": "GB/s", "frac": cap["dram_bytes"] / t_dom / 1e9 / peak}}
 
     # ---- end to end through the C ABI with host buffers -------------------------------------------------------
     host_in = torch.empty((L, L), dtype=torch.uint8).pin_memory()
@@ -319,7 +378,8 @@ def main():
         Ls, ns_sw = min(L, 4096), 12     # ~15 s of one host core at ~70 ns per spin
         ns, dt = oracle_ns_per_spin(Ls, q, w.model, w.T, w.seed, ns_sw, 1)
         cpu = {"value": ns, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"{ns_sw} oracle sweeps of an L={Ls} lattice of the same model and T after 1 warm-up sweep ({dt:.1f} s)"}
+               "sample": f"{ns_sw} oracle sweeps of an L={Ls} lattice of the same model and T after 1 warm-up sweep ({dt:.1f} s)",
+               "note": "the test oracle as it stands: single thread, never tuned (a checker, not a CPU Swendsen-Wang implementation to beat)"}
 
     if rank == 0:
         sweep_gbs = B_ALG * N / (total_ms / args.steps * 1e-3) / 1e9
@@ -329,7 +389,8 @@ def main():
             "dtype": "u8 spins / int32 labels / u32 Philox", "data": "synthetic",
             "config": {"workload": w.name, "L": L, "q": q, "model": "potts" if w.model == 0 else "clock", "T": w.T,
                        "equil_sweeps": args.equil, "l2": "flushed between steps (256 MiB memset, untimed)",
-                       "parallelism": "replicas only" if world > 1 else "single GPU", "backend": "tiled" if lat.algorithm == 2 else "generic"},
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "backend": {1: "generic", 2: "tiled", 3: "one CTA", 4: "hawick (paper)", 5: "kalentev (paper)"}[lat.algorithm]},
             "spin_flips_per_s": flips / (total_ms * 1e-3),
             "back_to_back": {"ns_per_spin_flip": b2b_ms * 1e6 / flips, "ms_per_step": b2b_ms / args.steps, "note": "same K sweeps in one enqueue, warm L2"},
             "with_measurement": {"ns_per_spin_flip": meas_ms * 1e6 / (args.steps * N), "ms_per_step": meas_ms / args.steps,
@@ -337,13 +398,12 @@ def main():
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N, "d2h_bytes_per_step": N + 2 * 16 * 8, "steps": e2e_steps},
             "gpu_launches": int(launches),
-            "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": traffic, "peak_source": peak_src, "ms_per_launch": prof[dom],
-                         "algorithmic_bytes_per_launch": dom_bytes},
-            "sweep_roofline": {"bytes_per_spin": B_ALG, "achieved_gbs": sweep_gbs, "frac": sweep_gbs / peak},
-            "issue_roofline": issue,
+            "roofline": roofline,
+            "sweep_roofline": {"bytes_per_spin": B_ALG, "achieved_gbs": sweep_gbs, "frac": sweep_gbs / peak,
+                               "note": "whole sweep at the contract's 10 B per spin (SURVEY 8(d)) against the measured HBM copy peak"},
             "kernels_ms": prof,
             "cpu_baseline": cpu,
+            "labeling_iterations_per_sweep": iters_per_sweep,
             "paper_context": {"gtx580_ns_per_spin_flip": 2.51, "source": "PAPER.md:83 Table 1 (another machine: context, not the target)"},
             "wall_s": wall,
         }

@@ -843,8 +843,11 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
 }
 
 // K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).  in = S^t, out = S^{t+1}.
+#ifndef SW_FLIP_MINB
+#define SW_FLIP_MINB 1
+#endif
 template <int MODEL, bool BATCH>
-__global__ void __launch_bounds__(TILE_THREADS)
+__global__ void __launch_bounds__(TILE_THREADS, SW_FLIP_MINB)
 k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsigned long long *parent, const uint32_t *ocount,
             const uint8_t *in, uint8_t *out, BatchView bv)
 {
