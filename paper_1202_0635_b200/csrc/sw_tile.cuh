@@ -861,6 +861,7 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsi
     const uint32_t ltile = BATCH ? blockIdx.x - lat * bv.tiles_per_lattice : blockIdx.x;
     const uint32_t tx = ltile % tiles_x, ty = ltile / tiles_x;
     const uint32_t x0 = tx * TW, y0 = ty * TH;
+    pdl_prologue();   // before every global load, also those of the constant per-lattice keys (tests/test_abi.py reads the SASS)
     PhiloxKey key_lat;
     if (BATCH) {
         key_lat = bv.keys[lat];
@@ -870,7 +871,6 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsi
     }
     const PhiloxKey &key = BATCH ? key_lat : key_one;
 
-    pdl_prologue();
     // one decision per open root of the tile (S3; R5 CLUSTER stream), keyed on the site index of the root
     // of its cluster in the global union-find
     const uint32_t no = ocount[blockIdx.x];
