@@ -221,6 +221,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default=None, help="a key of workloads.CONFIGS (default: the headline config)")
+    ap.add_argument("--L", type=int, default=0, help="override the workload's lattice size (the L-scan of PAPER.md:75, Table 1)")
     ap.add_argument("--equil", type=int, default=300, help="untimed sweeps from the random start before warm-up")
     ap.add_argument("--algo", default="auto", choices=["auto", "generic", "tiled", "small", "hawick", "kalentev"],
                     help="labeling back-end (sw_set_algorithm); hawick / kalentev are the paper's own labellers (A/B reference)")
@@ -253,6 +254,9 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     w = CONFIGS[args.workload or HEADLINE]
+    if args.L > 0:
+        import dataclasses
+        w = dataclasses.replace(w, L=args.L, name=f"{w.name}@L={args.L}")
     L, q, N = w.L, w.q, w.L * w.L
     from paper_1202_0635_b200 import replicas
     seed = replicas.replica_seed(w.seed, rank)       # replicas only: every rank its own lattice
@@ -384,7 +388,7 @@ def main():
     if rank == 0:
         sweep_gbs = B_ALG * N / (total_ms / args.steps * 1e-3) / 1e9
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "metric": METRIC if w.name == HEADLINE else "ns per spin flip (full SW sweep)", "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms / args.steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "u8 spins / int32 labels / u32 Philox", "data": "synthetic",
             "config": {"workload": w.name, "L": L, "q": q, "model": "potts" if w.model == 0 else "clock", "T": w.T,
