@@ -64,6 +64,14 @@ __device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *map, u
                  : "memory");
 }
 
+// shared-memory atomic add written as PTX (one lane of a warp adds the warp's total)
+__device__ __forceinline__ uint32_t atoms_add(uint32_t *p, uint32_t v)
+{
+    uint32_t old;
+    asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(smem_u32(p)), "r"(v) : "memory");
+    return old;
+}
+
 constexpr int TW = 128;                 // sites per tile row = 4 words of 32
 constexpr int TH = 64;                  // rows per tile
 constexpr int NWORD = TW / 32;
@@ -76,12 +84,8 @@ constexpr int LAB_WORDS = TILE_SITES + TILE_SITES / 32;   // skewed tile-local i
 #ifndef SW_EDGE_CAP
 #define SW_EDGE_CAP 256   // tests build a variant with tiny lists to drive the overflow paths
 #endif
-#ifndef SW_RCAP
-#define SW_RCAP 512
-#endif
 constexpr int EDGE_CAP = SW_EDGE_CAP;           // union edges listed per warp (more are handled by their own thread)
 constexpr int NDEC = 16;               // decisions are < q <= 16
-constexpr int RCAP = SW_RCAP;               // closed roots listed per warp for the converged decision draw
 constexpr int DEC_BASE = 512;           // lab16 value DEC_BASE + d: "closed cluster, decision d" (= OCAP)
 constexpr int ECNT = 2 * TH + 2 * TW;     // edge labels exported per tile: left column, right column, top row, bottom row
 constexpr int OCAP = 512;               // open roots listed per tile (<= 128 + 64 + 128 + 64 boundary positions)
@@ -231,7 +235,7 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
     __shared__ uint32_t s_H[TH][NWORD];
     __shared__ uint32_t s_V[TH][NWORD];
     __shared__ uint32_t s_lab[LAB_WORDS];
-    __shared__ uint32_t s_nopen;
+    __shared__ uint32_t s_nroot, s_nopen;                           // closed roots listed / open roots registered so far
     // s_ew: phase A reads the TMA-staged spins of the tile from it (TILE_SITES bytes), phase B keeps the per-warp edge
     // lists in it ([warp][EDGE_CAP + 1], + dump slot): the two uses never overlap in time
     constexpr int EDGE_WORDS = (TILE_THREADS / 32) * (EDGE_CAP + 1);
@@ -273,9 +277,16 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         if (lane == 0u) atomicAdd(stats + 8 + (i), (unsigned long long)(now_ - ph_t)); \
         ph_t = now_;                                                                    \
     }
-    static_assert(2 * (EDGE_CAP + 1) >= RCAP, "closed-root list must fit the warp's edge list");
+    // tile-wide list of the closed roots for the balanced decision draw (16-bit entries in s_ew once B2 is done with the edge
+    // lists); tests build a variant with a tiny list (SW_RCAP) to drive the overflow path
+#ifdef SW_RCAP
+    constexpr int RLCAP = SW_RCAP;
+#else
+    constexpr int RLCAP = 2 * EW_WORDS;
+#endif
+    static_assert(RLCAP <= 2 * EW_WORDS, "root list must fit the storage of the edge lists");
     uint32_t m = 0u;
-    if (tid == 32u) s_nopen = 0u;
+    if (tid == 32u) { s_nroot = 0u; s_nopen = 0u; }
     if (OBS && tid < 2u) s_obs[tid] = 0u;
     uint32_t o_neq = 0u, o_one = 0u;
     (void)o_neq; (void)o_one; (void)s_obs;
@@ -557,22 +568,32 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
             if (a != 0xFFFFFFFFu) {
                 uint32_t p;
                 while ((p = vl[a] & LMASK) != a) a = p;
-                vl[a] = a | LOPEN;
+                // The first thread to mark a root registers it: node blockIdx.x * OCAP + pos of the global union-find, its
+                // own parent, key = (site, node); the root's entry gets its output value LOPEN | pos in the upper half.
+                // (Atomic ORs: other boundary sites of the cluster mark the same entry at the same time.)
+                const uint32_t old = atomicOr(&s_lab[a], LOPEN);
+                if (!(old & LOPEN)) {
+                    const uint32_t pos = atomicAdd(&s_nopen, 1u);
+                    const uint32_t node = blockIdx.x * (uint32_t)OCAP + pos;
+                    parent[node] = ((unsigned long long)root_site(a, x0, y0, L) << 32) | node;
+                    atomicOr(&s_lab[a], (LOPEN | pos) << 16);
+                }
             }
         }
     }
     __syncthreads();
 
     SW_PHASE(4)
-    // B3b: the roots of the tile (S3 for the clusters that end inside the tile).  Only a run without a bond to the
-    // row above can be a root: every other run was given a smaller parent in B1.  `cand` = END bits of such runs
-    // (a carry started at the run start runs along the links of the run while no site has an up-bond and lands on
-    // the end bit).  A root's entry gets its final 16-bit output value in the upper half: open roots sp | LOPEN
-    // (they also join the tile's open list and the global union-find), closed roots DEC_BASE + decision, drawn from
-    // the CLUSTER stream keyed on the root's global site index (R5).
+    // B3b: the closed roots of the tile (S3 for the clusters that end inside the tile).  Only a run without a bond to the
+    // row above can be a root: every other run was given a smaller parent in B1.  `cand` = start bits of such runs.
+    // A closed root's entry gets its final 16-bit output value DEC_BASE + decision in the upper half, drawn from the
+    // CLUSTER stream keyed on the root's global site index (R5); the open roots got theirs,
+    // LOPEN | pos, in B3.
+    uint32_t mine = 0u;                           // this word's closed roots that did not fit the tile's list
+    uint16_t *const rl = reinterpret_cast<uint16_t *>(s_ew);
     {
         volatile uint32_t *vl = s_lab;
-        uint32_t rall = 0u;                       // this word's roots (their entries: sp, or sp | LOPEN when open)
+        uint32_t rall = 0u;                       // this word's roots
         uint32_t cand = cs;
         if (MODEL == 1) {
             // A spin on the mirror axis has no active bond at all (its thresholds are 0, R4) and the
@@ -599,62 +620,56 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
                 vl[sb + k] = (sb + k) | ((fuse ? (uint32_t)DEC_BASE : sb + k) << 16);
             }
         }
+        if (wy == 0u) cand = 0u;                  // every cluster with a site in the top row is open
         for (uint32_t c = cand; c;) {
             const uint32_t k = pop_top(c);
             const uint32_t v = vl[sb + k];
-            if ((v & LMASK) == sb + k) rall |= 1u << k;
+            if ((v & (LMASK | LOPEN)) == sb + k) rall |= 1u << k;     // a root, and not open
         }
-        // compact the warp's roots into its list (reusing the second half of the warp's edge list), so that the
-        // decisions are drawn -- and the open roots registered -- with all lanes busy
-        uint16_t *rl = reinterpret_cast<uint16_t *>(&s_edge[warp][0]) + 2 * (EDGE_CAP + 1) - RCAP;
-        const uint32_t n = __popc(rall);
+        // The closed roots of all warps go to one tile-wide list (16-bit entries in the storage of the edge lists, which
+        // B2 has left), so that after the barrier every thread takes one root per round and all warps carry the same
+        // load (the roots of a tile crowd in its upper rows).
+        const uint32_t n = (uint32_t)__popc(rall);
         uint32_t incl = n;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
             const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
             if (lane >= (uint32_t)d) incl += o;
         }
-        const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-        const bool listed = total <= (uint32_t)RCAP;
-        if (listed) {
-            uint32_t at = incl - n;
-            for (uint32_t rr = rall; rr;) {
-                const uint32_t k = pop_top(rr);
-                rl[at++] = (uint16_t)vl[sb + k];
-            }
-            __syncwarp();
+        uint32_t base = 0u;
+        if (lane == 31u) base = atoms_add(&s_nroot, incl);
+        uint32_t at = __shfl_sync(0xFFFFFFFFu, base, 31) + incl - n;
+        for (uint32_t rr = rall; rr;) {
+            const uint32_t k = pop_top(rr);
+            if (at < (uint32_t)RLCAP) rl[at] = (uint16_t)(sb + k);
+            else mine |= 1u << k;                 // hot configurations: more closed roots than the list holds
+            ++at;
         }
-        // listed: entry i of the warp's list; else (more roots than the list holds: hot configurations) every lane
-        // walks its own roots
-        uint32_t mine = rall;
-        for (uint32_t i = lane; listed ? (i < total) : (mine != 0u); i += 32u) {
-            uint32_t e;
-            if (listed) {
-                e = rl[i];
-            } else {
-                const uint32_t k = pop_top(mine);
-                e = vl[sb + k] & 0xFFFFu;
-            }
-            const uint32_t sp = e & LMASK;
-            const uint32_t r = root_site(sp, x0, y0, L);
-            uint32_t out = e;
-            if (e & LOPEN) {
-                // open root: node blockIdx.x * OCAP + pos of the global union-find, its own parent; key = (site, node)
-                const uint32_t pos = atomicAdd(&s_nopen, 1u);
-                const uint32_t node = blockIdx.x * (uint32_t)OCAP + pos;
-                parent[node] = ((unsigned long long)r << 32) | node;
-                out = LOPEN | pos;
-            } else if (fuse) {
+    }
+    __syncthreads();
+    {
+        volatile uint32_t *vl = s_lab;
+        if (tid == 0u) ocount[blockIdx.x] = s_nopen;
+        // closed roots: decision from the CLUSTER stream keyed on the root's global site index
+        auto decide = [&](uint32_t sp) {
+            uint32_t out = sp;
+            if (fuse) {
+                const uint32_t r = root_site(sp, x0, y0, L);
                 uint32_t w[4];
                 philox_stream<STREAM_CLUSTER, SW_K1_HILO>(key, r >> 2, t, w);
                 const uint32_t wsel = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
                 out = (uint32_t)DEC_BASE + (MODEL == 0 ? mulhi_q(wsel, (uint32_t)md.q) : (wsel >> 31));
             }
             vl[sp] = sp | (out << 16);
+        };
+        const uint32_t nc0 = s_nroot, nc = nc0 < (uint32_t)RLCAP ? nc0 : (uint32_t)RLCAP;
+        for (uint32_t i = tid; i < nc; i += TILE_THREADS) decide(rl[i]);
+        while (mine) {
+            const uint32_t k = pop_top(mine);
+            decide(sb + k);
         }
     }
     __syncthreads();
-    if (tid == 0u) ocount[blockIdx.x] = s_nopen;
 
     SW_PHASE(7)
     // B4a: resolve every run of the word to its root's entry (whose upper half is the output value).  Two runs at
