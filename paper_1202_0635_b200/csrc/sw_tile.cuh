@@ -124,13 +124,26 @@ static inline size_t tiled_workspace_bytes_n(int L, size_t nlat);
 static inline size_t tiled_workspace_bytes(int L) { return tiled_workspace_bytes_n(L, 1); }
 
 // ---- shared-memory union-find by minimum index (same scheme as uf_union in sw_generic.cuh) ------------------
-__device__ __forceinline__ uint32_t sfind_halve(volatile uint32_t *lab, uint32_t a)
+// Labels in shared memory are BYTE OFFSETS into the label array (4 x the skewed tile-local index): a hop is then one
+// LDS with the pointer as its address, no mask, no shift.  The low 16 bits of an entry hold the pointer (the entry's own
+// offset for a root), the high 16 bits stay 0 until the cluster's output value is known (phases B3, B3b).
+__device__ __forceinline__ uint32_t lab_ld(const char *lab, uint32_t off) { return *reinterpret_cast<const volatile uint32_t *>(lab + off); }
+__device__ __forceinline__ uint32_t ptr_ld(const char *lab, uint32_t off)
 {
-    uint32_t cur = lab[a];
+    // the 16-bit pointer field, zero-extended (PTX, so that the compiler keeps plain 32-bit compares on the result)
+    uint32_t v;
+    asm volatile("ld.volatile.shared.u16 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(lab) + off) : "memory");
+    return v;
+}
+__device__ __forceinline__ void lab_st(char *lab, uint32_t off, uint32_t v) { *reinterpret_cast<volatile uint32_t *>(lab + off) = v; }
+
+__device__ __forceinline__ uint32_t sfind_halve(char *lab, uint32_t a)
+{
+    uint32_t cur = lab_ld(lab, a);
     if (cur != a) {
         uint32_t prev = a, next;
-        while (cur > (next = lab[cur])) {
-            lab[prev] = next;
+        while (cur > (next = lab_ld(lab, cur))) {
+            lab_st(lab, prev, next);
             prev = cur;
             cur = next;
         }
@@ -138,14 +151,14 @@ __device__ __forceinline__ uint32_t sfind_halve(volatile uint32_t *lab, uint32_t
     return cur;
 }
 
-__device__ __forceinline__ void sunion(uint32_t *lab, uint32_t a, uint32_t b)
+__device__ __forceinline__ void sunion(char *lab, uint32_t a, uint32_t b)
 {
     for (;;) {
         a = sfind_halve(lab, a);
         b = sfind_halve(lab, b);
         if (a == b) return;
         if (a < b) { const uint32_t tmp = a; a = b; b = tmp; }
-        const uint32_t old = atomicMin(lab + a, b);   // a > b
+        const uint32_t old = atomicMin(reinterpret_cast<uint32_t *>(lab + a), b);   // a > b
         if (old == a) return;
         a = old;
     }
@@ -163,14 +176,21 @@ __device__ __forceinline__ uint32_t pop_top(uint32_t &c)
     const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
     c &= c - 1u;
 #else
-    const uint32_t k = 31u - (uint32_t)__clz((int)c);
+    const uint32_t k = top_bit(c);
     c ^= 1u << k;
 #endif
     return k;
 }
 
+// position of the highest set bit (x != 0): one FLO (31 - __clz(x) compiles to FLO + a subtraction that is then undone)
+__device__ __forceinline__ uint32_t top_bit(uint32_t x)
+{
+    uint32_t r;
+    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+    return r;
+}
 // first site (bit position) of the segment that holds bit k; S = mask of segment starts (bit 0 always set)
-__device__ __forceinline__ uint32_t seg_start(uint32_t S, uint32_t k) { return 31u - __clz(S & ((2u << k) - 1u)); }
+__device__ __forceinline__ uint32_t seg_start(uint32_t S, uint32_t k) { return top_bit(S & ((2u << k) - 1u)); }
 
 // Global site index of the tile-local root named by label word `v` of a site of the tile with origin (X0, Y0).
 __device__ __forceinline__ uint32_t root_site(uint32_t v, uint32_t X0, uint32_t Y0, uint32_t L)
@@ -395,11 +415,14 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
     if (tid < (uint32_t)NWORD) vedge[(size_t)ty * (L / 32) + (x0 >> 5) + tid] = s_V[TH - 1][tid];
 
     // ---------------- phase B: one thread per word --------------------------------------------------------
-    // All label values are SKEWED tile-local indices sp = p + (p >> 5) (one pad word per 32-site word), so that the
-    // 32 lanes of a warp, which own 32 different words, hit 32 different banks when they touch the same bit position.
+    // Label entries are addressed by SKEWED tile-local indices sp = p + (p >> 5) (one pad word per 32-site word), so that
+    // the 32 lanes of a warp, which own 32 different words, hit 32 different banks when they touch the same bit position;
+    // what is stored and passed around is the BYTE OFFSET 4 sp of an entry (see lab_ld above).
+    char *const lab = reinterpret_cast<char *>(s_lab);
+    constexpr uint32_t OPENBIT = 0x80000000u;                 // entry of a root of an open cluster (= LOPEN of its output value)
     const uint32_t wy = tid / NWORD, ww = tid % NWORD;
-    const uint32_t sb = 33u * tid;                            // skewed index of the word's first site
-    const uint32_t sbu = sb - 132u;                           // ... of the word above (tid - 4)
+    const uint32_t sb = 132u * tid;                           // offset of the entry of the word's first site
+    const uint32_t sbu = sb - 528u;                           // ... of the word above (tid - 4)
     const uint32_t h = s_H[wy][ww];
     const uint32_t hin = h & 0x7FFFFFFFu;                     // bonds inside the word
     const uint32_t S = ~(hin << 1);                           // run starts (bit 0 always)
@@ -448,19 +471,24 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         uint32_t *el = s_edge[warp];
         for (uint32_t c = cs; c;) {
             const uint32_t k = pop_top(c);
-            s_lab[sb + k] = sb + k;
+            lab_st(lab, sb + 4u * k, sb + 4u * k);
         }
-        for (uint32_t f = first; f;) {
-            const uint32_t k = pop_top(f);
-            s_lab[sb + seg_start(S, k)] = sbu + seg_start(Sa, k);
+        // `first` and the start bits of the runs that have an up-bond (S & ~cs) hold one bit per such run, in the same
+        // order: both are walked from the top, so the run's start needs no search
+        for (uint32_t f = first, fs = S & ~cs; f;) {
+            const uint32_t k = top_bit(f), ks = top_bit(fs);
+            const uint32_t bit = 1u << k;
+            f ^= bit;
+            fs ^= 1u << ks;
+            lab_st(lab, sb + 4u * ks, sbu + 4u * top_bit(Sa & (2u * bit - 1u)));
         }
         for (uint32_t xr = X; xr;) {
             const uint32_t k = pop_top(xr);
-            if (epos < (uint32_t)EDGE_CAP) el[epos] = (sb + seg_start(S, k)) | ((sbu + seg_start(Sa, k)) << 16);
+            if (epos < (uint32_t)EDGE_CAP) el[epos] = (sb + 4u * seg_start(S, k)) | ((sbu + 4u * seg_start(Sa, k)) << 16);
             ++epos;
         }
         if (hedge_out) {                                      // bond to the next word of the row
-            if (epos < (uint32_t)EDGE_CAP) el[epos] = (sb + 33u) | ((sb + seg_start(S, 31u)) << 16);
+            if (epos < (uint32_t)EDGE_CAP) el[epos] = (sb + 132u) | ((sb + 4u * seg_start(S, 31u)) << 16);
             ++epos;
         }
     }
@@ -469,36 +497,10 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
 #ifndef SW_RESOLVE_PASSES
 #define SW_RESOLVE_PASSES 2
 #endif
-#ifndef SW_JUMP_ROUNDS
-#define SW_JUMP_ROUNDS 0
-#endif
-    // B1b: pointer jumping on the inheritance forest (plain stores only so far: any ancestor is a valid parent, so the
-    // rounds need no barrier between them).  Shallow trees make the finds of B2 and the resolve pass of B4a short.
-#pragma unroll 1
-    for (int r = 0; r < SW_JUMP_ROUNDS; ++r) {
-        volatile uint32_t *vl = s_lab;
-        uint32_t sr = S & ~cs;                                 // runs that inherited
-        while (sr) {
-            uint32_t kk[4], x[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                kk[j] = sr ? (uint32_t)__ffs((int)sr) - 1u : kk[0];
-                sr &= sr - 1u;
-            }
-#pragma unroll
-            for (int j = 0; j < 4; ++j) x[j] = vl[sb + kk[j]];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) x[j] = vl[x[j]];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) vl[sb + kk[j]] = x[j];
-        }
-    }
-    if (SW_JUMP_ROUNDS > 0) __syncthreads();
 
     // B2: the warp's edges, one per lane and round (union-find by minimum index: PAPER.md:47 at tile level)
     {
         const uint32_t ne = etotal < (uint32_t)EDGE_CAP ? etotal : (uint32_t)EDGE_CAP;
-        volatile uint32_t *vl = s_lab;
         // One edge in flight per lane; a lane that has merged its edge takes the next unclaimed one of the warp's
         // list at once (shared counter), so no lane waits for the slowest edge of a batch.
         {
@@ -506,18 +508,18 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
             bool have = e < ne;
             if (have) { const uint32_t v = s_edge[warp][e]; ea = v & 0xFFFFu; eb = v >> 16; }
             while (have) {
-                const uint32_t pa = vl[ea], pb = vl[eb];
-                const uint32_t ga = vl[pa], gb = vl[pb];
+                const uint32_t pa = lab_ld(lab, ea), pb = lab_ld(lab, eb);
+                const uint32_t ga = lab_ld(lab, pa), gb = lab_ld(lab, pb);
                 bool done = false;
                 if (pa != ea || pb != eb) {
-                    if (ga != pa) vl[ea] = ga;                   // path halving: skip one ancestor on each side
-                    if (gb != pb) vl[eb] = gb;
+                    if (ga != pa) lab_st(lab, ea, ga);           // path halving: skip one ancestor on each side
+                    if (gb != pb) lab_st(lab, eb, gb);
                     ea = ga; eb = gb;
                 } else if (ea == eb) {
                     done = true;
                 } else {
                     const uint32_t hi = ea > eb ? ea : eb, lo = ea > eb ? eb : ea;
-                    const uint32_t old = atomicMin(s_lab + hi, lo);
+                    const uint32_t old = atomicMin(reinterpret_cast<uint32_t *>(lab + hi), lo);
                     if (old == hi) done = true;
                     else { ea = old; eb = lo; }                  // hi had a parent already: keep it connected to lo
                 }
@@ -533,10 +535,10 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
             uint32_t slot = epos0, Xr = X;
             while (Xr) {
                 const uint32_t k = pop_top(Xr);
-                if (slot >= (uint32_t)EDGE_CAP) sunion(s_lab, sb + seg_start(S, k), sbu + seg_start(Sa, k));
+                if (slot >= (uint32_t)EDGE_CAP) sunion(lab, sb + 4u * seg_start(S, k), sbu + 4u * seg_start(Sa, k));
                 ++slot;
             }
-            if (hedge_out && slot >= (uint32_t)EDGE_CAP) sunion(s_lab, sb + 33u, sb + seg_start(S, 31u));
+            if (hedge_out && slot >= (uint32_t)EDGE_CAP) sunion(lab, sb + 132u, sb + 4u * seg_start(S, 31u));
         }
     }
     __syncthreads();
@@ -546,37 +548,36 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
     // (their bonds belong to the neighbouring tiles), or with an active bond across the right or bottom edge.
     // One boundary site per thread and pass; only the first site of a run (or of a bonded stretch) does the work.
     {
-        volatile uint32_t *vl = s_lab;
         uint32_t c0 = 0xFFFFFFFFu, c1 = 0xFFFFFFFFu;
         if (tid < (uint32_t)TW) {
             const uint32_t w = tid >> 5, k = tid & 31u;
             const uint32_t S0 = ~((s_H[0][w] & 0x7FFFFFFFu) << 1);
-            if ((S0 >> k) & 1u) c0 = 33u * w + k;
+            if ((S0 >> k) & 1u) c0 = 4u * (33u * w + k);
             const uint32_t hb = s_H[TH - 1][w] & 0x7FFFFFFFu, vb = s_V[TH - 1][w];
             const bool dup = k > 0u && ((vb & hb) >> (k - 1u)) & 1u;
-            if (((vb >> k) & 1u) && !dup) c1 = 33u * ((TH - 1) * NWORD + w) + seg_start(~(hb << 1), k);
+            if (((vb >> k) & 1u) && !dup) c1 = 4u * (33u * ((TH - 1) * NWORD + w) + seg_start(~(hb << 1), k));
         } else if (tid < (uint32_t)(TW + TH)) {
-            c0 = 33u * ((tid - TW) * NWORD);
+            c0 = 4u * (33u * ((tid - TW) * NWORD));
         } else if (tid < (uint32_t)(TW + 2 * TH)) {
             const uint32_t r = tid - (TW + TH);
             const uint32_t hr = s_H[r][NWORD - 1];
-            if (hr >> 31) c0 = 33u * (r * NWORD + NWORD - 1) + seg_start(~((hr & 0x7FFFFFFFu) << 1), 31u);
+            if (hr >> 31) c0 = 4u * (33u * (r * NWORD + NWORD - 1) + seg_start(~((hr & 0x7FFFFFFFu) << 1), 31u));
         }
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
             uint32_t a = c ? c1 : c0;
             if (a != 0xFFFFFFFFu) {
                 uint32_t p;
-                while ((p = vl[a] & LMASK) != a) a = p;
+                while ((p = ptr_ld(lab, a)) != a) a = p;
                 // The first thread to mark a root registers it: node blockIdx.x * OCAP + pos of the global union-find, its
                 // own parent, key = (site, node); the root's entry gets its output value LOPEN | pos in the upper half.
                 // (Atomic ORs: other boundary sites of the cluster mark the same entry at the same time.)
-                const uint32_t old = atomicOr(&s_lab[a], LOPEN);
-                if (!(old & LOPEN)) {
+                const uint32_t old = atomicOr(reinterpret_cast<uint32_t *>(lab + a), OPENBIT);
+                if (!(old & OPENBIT)) {
                     const uint32_t pos = atomicAdd(&s_nopen, 1u);
                     const uint32_t node = blockIdx.x * (uint32_t)OCAP + pos;
-                    parent[node] = ((unsigned long long)root_site(a, x0, y0, L) << 32) | node;
-                    atomicOr(&s_lab[a], (LOPEN | pos) << 16);
+                    parent[node] = ((unsigned long long)root_site(a >> 2, x0, y0, L) << 32) | node;
+                    atomicOr(reinterpret_cast<uint32_t *>(lab + a), pos << 16);
                 }
             }
         }
@@ -589,11 +590,10 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
     // A closed root's entry gets its final 16-bit output value DEC_BASE + decision in the upper half, drawn from the
     // CLUSTER stream keyed on the root's global site index (R5); the open roots got theirs,
     // LOPEN | pos, in B3.
-    uint32_t mine = 0u;                           // this word's closed roots that did not fit the tile's list
+    uint32_t mine = 0u;                           // this word's closed roots that did not fit
     uint16_t *const rl = reinterpret_cast<uint16_t *>(s_ew);
     {
-        volatile uint32_t *vl = s_lab;
-        uint32_t rall = 0u;                       // this word's roots
+        uint32_t rall = 0u;                       // this word's closed roots
         uint32_t cand = cs;
         if (MODEL == 1) {
             // A spin on the mirror axis has no active bond at all (its thresholds are 0, R4) and the
@@ -615,16 +615,15 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
                 ax |= ((z * 0x00204081u) >> 28) << (4 * j);          // bits 7, 15, 23, 31 -> one nibble
             }
             cand &= ~ax;
-            while (ax) {
+            while (ax) {                          // (also when B3 marked it open: it has no bond at all, so it is closed)
                 const uint32_t k = pop_top(ax);
-                vl[sb + k] = (sb + k) | ((fuse ? (uint32_t)DEC_BASE : sb + k) << 16);
+                lab_st(lab, sb + 4u * k, (sb + 4u * k) | ((fuse ? (uint32_t)DEC_BASE : (sb >> 2) + k) << 16));
             }
         }
         if (wy == 0u) cand = 0u;                  // every cluster with a site in the top row is open
         for (uint32_t c = cand; c;) {
             const uint32_t k = pop_top(c);
-            const uint32_t v = vl[sb + k];
-            if ((v & (LMASK | LOPEN)) == sb + k) rall |= 1u << k;     // a root, and not open
+            if (lab_ld(lab, sb + 4u * k) == sb + 4u * k) rall |= 1u << k;     // a root, and not open (upper half still 0)
         }
         // The closed roots of all warps go to one tile-wide list (16-bit entries in the storage of the edge lists, which
         // B2 has left), so that after the barrier every thread takes one root per round and all warps carry the same
@@ -641,17 +640,16 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         uint32_t at = __shfl_sync(0xFFFFFFFFu, base, 31) + incl - n;
         for (uint32_t rr = rall; rr;) {
             const uint32_t k = pop_top(rr);
-            if (at < (uint32_t)RLCAP) rl[at] = (uint16_t)(sb + k);
+            if (at < (uint32_t)RLCAP) rl[at] = (uint16_t)(sb + 4u * k);
             else mine |= 1u << k;                 // hot configurations: more closed roots than the list holds
             ++at;
         }
     }
     __syncthreads();
     {
-        volatile uint32_t *vl = s_lab;
         if (tid == 0u) ocount[blockIdx.x] = s_nopen;
-        // closed roots: decision from the CLUSTER stream keyed on the root's global site index
-        auto decide = [&](uint32_t sp) {
+        auto decide = [&](uint32_t o) {           // o = offset of the entry of a closed root
+            const uint32_t sp = o >> 2;
             uint32_t out = sp;
             if (fuse) {
                 const uint32_t r = root_site(sp, x0, y0, L);
@@ -660,45 +658,39 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
                 const uint32_t wsel = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
                 out = (uint32_t)DEC_BASE + (MODEL == 0 ? mulhi_q(wsel, (uint32_t)md.q) : (wsel >> 31));
             }
-            vl[sp] = sp | (out << 16);
+            lab_st(lab, o, o | (out << 16));
         };
         const uint32_t nc0 = s_nroot, nc = nc0 < (uint32_t)RLCAP ? nc0 : (uint32_t)RLCAP;
         for (uint32_t i = tid; i < nc; i += TILE_THREADS) decide(rl[i]);
         while (mine) {
             const uint32_t k = pop_top(mine);
-            decide(sb + k);
+            decide(sb + 4u * k);
         }
     }
     __syncthreads();
 
     SW_PHASE(7)
     // B4a: resolve every run of the word to its root's entry (whose upper half is the output value).  Two runs at
-    // a time, three pointer hops each (the loads of one level are independent, so their latencies overlap), result
-    // written back to the run's own entry; runs deeper than that (rare) are finished by a chase that starts from the
-    // already advanced pointer.
+    // a time, three pointer hops each (the loads of one level are independent, so their latencies overlap; the first two
+    // read the 16-bit pointer only), result written back to the run's own entry; runs deeper than that (rare) are
+    // finished by a chase that starts from the already advanced pointer.
     uint32_t hops = 0u;
     {
-        volatile uint32_t *vl = s_lab;
         // one pass over the runs in `todo`: returns the runs that are still not at their root
         auto pass = [&](uint32_t todo) -> uint32_t {
             uint32_t rem = 0u;
             while (todo) {
                 // the lowest and the highest run still to do (the same run when one is left: harmless repeat)
-#ifndef SW_CLZ_LOOPS
-                const uint32_t k0 = (uint32_t)__ffs((int)todo) - 1u, k1 = 31u - (uint32_t)__clz((int)todo);
+                const uint32_t k0 = (uint32_t)__ffs((int)todo) - 1u, k1 = top_bit(todo);
                 todo &= todo - 1u;
                 todo &= ~(1u << k1);
-#else
-                const uint32_t k1 = pop_top(todo);
-                const uint32_t k0 = todo ? pop_top(todo) : k1;
-#endif
-                uint32_t x0 = vl[sb + k0], x1 = vl[sb + k1];
-                x0 = vl[x0 & LMASK]; x1 = vl[x1 & LMASK];
-                const uint32_t y0r = vl[x0 & LMASK], y1r = vl[x1 & LMASK];
-                vl[sb + k0] = y0r;
-                vl[sb + k1] = y1r;
-                if ((y0r ^ x0) & LMASK) rem |= 1u << k0;
-                if ((y1r ^ x1) & LMASK) rem |= 1u << k1;
+                uint32_t x0 = ptr_ld(lab, sb + 4u * k0), x1 = ptr_ld(lab, sb + 4u * k1);
+                x0 = ptr_ld(lab, x0); x1 = ptr_ld(lab, x1);
+                const uint32_t y0r = lab_ld(lab, x0), y1r = lab_ld(lab, x1);
+                lab_st(lab, sb + 4u * k0, y0r);
+                lab_st(lab, sb + 4u * k1, y1r);
+                if ((y0r ^ x0) & 0xFFFCu) rem |= 1u << k0;         // pointer fields differ (offsets are multiples of 4)
+                if ((y1r ^ x1) & 0xFFFCu) rem |= 1u << k1;
             }
             return rem;
         };
@@ -706,11 +698,11 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
 #pragma unroll 1
         for (int r = 0; r < SW_RESOLVE_PASSES - 1; ++r) rem = pass(rem);   // the written-back pointers of all runs shorten these
         while (rem) {
-            const uint32_t k = 31u - (uint32_t)__clz((int)rem);
+            const uint32_t k = top_bit(rem);
             rem ^= 1u << k;
-            uint32_t a = vl[sb + k] & LMASK, v;
-            while (((v = vl[a]) & LMASK) != a) { a = v & LMASK; ++hops; }
-            vl[sb + k] = v;
+            uint32_t a = ptr_ld(lab, sb + 4u * k), p;
+            while ((p = ptr_ld(lab, a)) != a) { a = p; ++hops; }
+            lab_st(lab, sb + 4u * k, lab_ld(lab, a));
         }
     }
     __syncwarp();
@@ -718,10 +710,9 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
 
     // B4b: per-site labels of the word (64 contiguous bytes)
     {
-        volatile uint32_t *vl = s_lab;
         uint32_t xs[32];
 #pragma unroll
-        for (int k = 0; k < 32; ++k) xs[k] = ((S >> k) & 1u) ? vl[sb + k] : 0u;
+        for (int k = 0; k < 32; ++k) xs[k] = ((S >> k) & 1u) ? lab_ld(lab, sb + 4u * k) : 0u;
         uint32_t cur = 0u, o[16];
 #pragma unroll
         for (int k = 0; k < 32; ++k) {
