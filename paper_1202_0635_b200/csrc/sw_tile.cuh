@@ -10,9 +10,11 @@
 //                 above its lowest such bond; B2: only the remaining, non-redundant up-bonds and the bonds between
 //                 words go through the shared-memory union-find (atomicMin, root = smallest index: the "proper
 //                 label ... smallest" of PAPER.md:47 at tile level); B3: clusters that may continue in another
-//                 tile are marked open; B3b: every closed root draws its cluster's decision (CLUSTER stream keyed
-//                 on its global site index), every open root becomes node tile * OCAP + pos of the global
-//                 union-find; B4: every run resolves to its root.
+//                 tile are marked open by their boundary sites, and the first thread to mark a root registers it as
+//                 node tile * OCAP + pos of the global union-find; B3b: the closed roots of all warps are listed
+//                 tile-wide and every thread draws one cluster decision per round (CLUSTER stream keyed on the root's
+//                 global site index); B4: every run resolves to its root.  Labels in shared memory are byte offsets
+//                 (a pointer hop is one LDS), the pointer in the low half of an entry, the output value in the high half.
 //        output   one uint16 per site: DEC_BASE + decision (closed cluster) or LOPEN | pos (open cluster); the labels
 //                 of the tile's boundary sites also go to a compact edge array for K2.
 //   K2 k_seam_merge   S2b: union across every active tile-crossing bond in the global union-find over open roots
@@ -170,6 +172,13 @@ __device__ __forceinline__ void sunion(char *lab, uint32_t a, uint32_t b)
 #ifndef SW_K1_HILO
 #define SW_K1_HILO 0u
 #endif
+// position of the highest set bit (x != 0): one FLO (31 - __clz(x) compiles to FLO + a subtraction that is then undone)
+__device__ __forceinline__ uint32_t top_bit(uint32_t x)
+{
+    uint32_t r;
+    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+    return r;
+}
 __device__ __forceinline__ uint32_t pop_top(uint32_t &c)
 {
 #ifndef SW_CLZ_LOOPS
@@ -182,13 +191,6 @@ __device__ __forceinline__ uint32_t pop_top(uint32_t &c)
     return k;
 }
 
-// position of the highest set bit (x != 0): one FLO (31 - __clz(x) compiles to FLO + a subtraction that is then undone)
-__device__ __forceinline__ uint32_t top_bit(uint32_t x)
-{
-    uint32_t r;
-    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
-    return r;
-}
 // first site (bit position) of the segment that holds bit k; S = mask of segment starts (bit 0 always set)
 __device__ __forceinline__ uint32_t seg_start(uint32_t S, uint32_t k) { return top_bit(S & ((2u << k) - 1u)); }
 
