@@ -77,16 +77,18 @@ def num(vals, k):
 
 
 def read_source(rep: str):
-    """-> list of (file, line, opcode, warp instructions executed, {stall: samples}, samples)."""
+    """-> list of (file, line, opcode, warp instructions executed, {stall: samples}, samples, SASS address, thread
+    instructions executed), in SASS address order."""
     src = subprocess.run(["ncu", "-i", rep, "--page", "source", "--csv", "--print-source", "cuda,sass"], capture_output=True, text=True, check=True).stdout
     out, cur, line, h = [], None, None, None
+    seen = set()       # an instruction inlined from a helper is listed under every source line of its inline chain: count it once
     for r in csv.reader(src.splitlines()):
         if r and r[0] == "File Path":
             cur = r[1].split("/")[-1]
             continue
         if r and r[0] == "Line No":
             h = r
-            ii, si = h.index("Instructions Executed"), h.index("# Samples")
+            ii, si, ti = h.index("Instructions Executed"), h.index("# Samples"), h.index("Thread Instructions Executed")
             st = {n[6:]: h.index(n) for n in h if n.startswith("stall_") and "Not Issued" not in n}
             continue
         if not r or h is None:
@@ -100,6 +102,9 @@ def read_source(rep: str):
             except ValueError:
                 continue
             m = re.match(r"\s*(@!?U?P\d+\s+)?([A-Z0-9_.]+)", r[3])
+            if m and r[2] in seen:
+                continue
+            seen.add(r[2])
             if m:
                 stalls = {}
                 for k, ix in st.items():
@@ -107,7 +112,8 @@ def read_source(rep: str):
                         stalls[k] = int(r[ix] or 0)
                     except ValueError:
                         pass
-                out.append((cur, line, m.group(2), n, stalls, int(r[si] or 0)))
+                out.append((cur, line, m.group(2), n, stalls, int(r[si] or 0), int(r[2], 16), int(r[ti] or 0)))
+    out.sort(key=lambda t: t[6])          # SASS address order
     return out
 
 
@@ -137,7 +143,7 @@ def main():
     ops = collections.Counter()
     cls = collections.Counter()
     busy = collections.Counter()
-    for _, _, op, n, _, _ in rows:
+    for _, _, op, n, _, _, _, _ in rows:
         c, b = classify(op)
         ops["IMAD.WIDE" if c == "imad_wide" else "IMAD.HI" if c == "imad_hi" else op.split(".")[0]] += n
         cls[c] += n
@@ -169,22 +175,27 @@ def main():
             a, b = rng.split("-")
             ph.append((int(a), int(b), name))
         agg = collections.defaultdict(collections.Counter)
-        for f, line, op, n, stalls, smp in rows:
-            key = "philox" if f == "sw_philox.cuh" else next((nm for a, b, nm in ph if f == fname and a <= line <= b), "other")
+        # in SASS address order; an instruction inlined from a helper (Philox, bit scans, label loads) belongs to the phase
+        # of the nearest preceding instruction that maps to a line of FILE itself
+        key = "prologue"
+        for f, line, op, n, stalls, smp, _, tn in rows:
+            if f == fname:
+                key = next((nm for a, b, nm in ph if a <= line <= b), key)
             a = agg[key]
             a["inst"] += n
+            a["thread_inst"] += tn
             a["samples"] += smp
             for pipe, cyc in classify(op)[1].items():
                 a[pipe] += cyc * n
             for k, v in stalls.items():
                 a["stall_" + k] += v
         tot_s = sum(a["samples"] for a in agg.values()) or 1
-        print("\n### by phase (source-line ranges): instructions, pipe cycles (M) and share of the warp-stall samples\n")
-        print("| phase | inst M | alu | fma | xu | lsu | samples | top stall reasons |\n|---|---|---|---|---|---|---|---|")
-        for k, a in sorted(agg.items(), key=lambda kv: -kv[1]["samples"]):
+        print("\n### by phase (source-line ranges of " + fname + ", SASS address order): instructions, active lanes, pipe cycles (M) and share of the warp-stall samples\n")
+        print("| phase | inst M | lanes | alu | fma | xu | lsu | samples | top stall reasons |\n|---|---|---|---|---|---|---|---|---|")
+        for k, a in agg.items():
             st = sorted(((n[6:], c) for n, c in a.items() if n.startswith("stall_")), key=lambda t: -t[1])[:4]
-            print(f"| {k} | {a['inst'] / 1e6:.2f} | {a['alu'] / 1e6:.1f} | {a['fma'] / 1e6:.1f} | {a['xu'] / 1e6:.1f} | {a['lsu'] / 1e6:.1f} | "
-                  f"{a['samples'] / tot_s:.3f} | " + ", ".join(f"{n} {c / max(1, a['samples']):.2f}" for n, c in st) + " |")
+            print(f"| {k} | {a['inst'] / 1e6:.2f} | {a['thread_inst'] / max(1, a['inst']):.1f} | {a['alu'] / 1e6:.1f} | {a['fma'] / 1e6:.1f} | {a['xu'] / 1e6:.1f} | "
+                  f"{a['lsu'] / 1e6:.1f} | {a['samples'] / tot_s:.3f} | " + ", ".join(f"{n} {c / max(1, a['samples']):.2f}" for n, c in st) + " |")
 
     if args.record:
         tj = ROOT / "profiles" / "traffic.json"
