@@ -73,7 +73,9 @@ void sw_destroy(sw_ctx *ctx);
 
 /* n >= 0 full SW sweeps (steps S0-S4 of DESIGN.md section 1), sweep indices
  * t .. t+n-1 where t = sw_sweep_index().  sw_sweep(a); sw_sweep(b) == sw_sweep(a+b).
- * sw_sweep returns after the work is complete; sw_sweep_async only enqueues it on the stream. */
+ * sw_sweep returns after the work is complete; sw_sweep_async only enqueues it on the stream.
+ * Tiled back-end: whole chunks of 16 sweeps are replayed from a CUDA graph (one cudaGraphLaunch per chunk instead of 48
+ * kernel launches; the environment variable SW_NO_GRAPH=1, read by sw_create*, turns that off); the result is the same. */
 int sw_sweep(sw_ctx *ctx, int n);
 int sw_sweep_async(sw_ctx *ctx, int n);
 int sw_sync(sw_ctx *ctx);

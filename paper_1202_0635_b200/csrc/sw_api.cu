@@ -107,6 +107,12 @@ struct sw_ctx {
     uint64_t ccl_iterations = 0, ccl_sweeps = 0;   // SW_ALGO_HAWICK / SW_ALGO_KALENTEV: scan passes and the sweeps they served
     sw::TiledState tiled{};
     unsigned long long *rec_host = nullptr;   // pinned copy of the record ring (sw_sweep_record)
+    // Tiled back-end: chunks of GRAPH_SWEEPS sweeps replayed from a CUDA graph (one per parity of the spin ping-pong);
+    // the kernels of a graph read the sweep index as "offset inside the chunk + *t_dev".
+    cudaGraphExec_t graph[2] = { nullptr, nullptr };
+    uint32_t *t_dev = nullptr;
+    uint64_t t_dev_value = ~0ull;             // what *t_dev holds (~0: unknown)
+    bool graph_off = false;                   // SW_NO_GRAPH=1, or capture failed once: plain launches from then on
 };
 
 namespace {
@@ -216,6 +222,59 @@ int generic_sweep(sw_ctx *c, uint32_t t, cudaEvent_t *ev)
 // obs_row (optional): zeroed row of the record ring that receives the observables of S^t if the back-end fuses S5 into
 // its first kernel (fuses_observables); otherwise the caller has launched k_observables on it already.
 bool fuses_observables(const sw_ctx *c) { return c->algo == SW_ALGO_TILED && sw::tiled_fuses_observables(c->md); }
+
+// sw_sweep(n) of the tiled back-end, n >= GRAPH_SWEEPS: the 3 kernels of GRAPH_SWEEPS consecutive sweeps (with their
+// programmatic-dependent-launch edges) are captured once per ping-pong parity and replayed with one cudaGraphLaunch per
+// chunk ("CUDA graph or persistent kernel" as the host scheduler).  GRAPH_SWEEPS is even, so a chunk leaves
+// the roles of the two spin buffers as it found them.
+constexpr int GRAPH_SWEEPS = 16;
+
+bool build_graph(sw_ctx *c, int which)
+{
+    // captured on a private stream (the context's may be the legacy default stream, which cannot capture); nothing runs
+    // on it: the instantiated graph is launched on the context's stream
+    cudaStream_t cap = nullptr;
+    if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); cudaStreamDestroy(cap); return false; }
+    uint8_t *a = c->spins, *b = c->spins_alt;
+    uint64_t dummy = 0;
+    bool ok = true;
+    for (int s = 0; s < GRAPH_SWEEPS && ok; ++s) {
+        ok = sw::tiled_sweep(c->tiled, c->md, c->key, (uint32_t)s, a, b, (unsigned long long *)c->labels, cap, nullptr, &dummy, nullptr,
+                             nullptr, c->t_dev) == 0;
+        std::swap(a, b);
+    }
+    ok = ok && sw::launch_pdl(sw::k_advance_t, 1u, 32u, cap, c->t_dev, (uint32_t)GRAPH_SWEEPS) == cudaSuccess;
+    cudaGraph_t g = nullptr;
+    if (cudaStreamEndCapture(cap, &g) != cudaSuccess || !g) ok = false;
+    cudaStreamDestroy(cap);
+    if (ok && cudaGraphInstantiate(&c->graph[which], g, 0) != cudaSuccess) { c->graph[which] = nullptr; ok = false; }
+    if (g) cudaGraphDestroy(g);
+    if (!ok) cudaGetLastError();
+    return ok;
+}
+
+// as many whole chunks of n sweeps as possible through the graphs; returns the number of sweeps done (0: none)
+int graph_sweeps(sw_ctx *c, int n)
+{
+    int done = 0;
+    while (n - done >= GRAPH_SWEEPS && !c->graph_off) {
+        const int which = c->spins == c->tiled.map_base[0] ? 0 : 1;
+        if (!c->graph[which] && !build_graph(c, which)) { c->graph_off = true; break; }
+        if (c->t_dev_value != c->t) {
+            sw::k_set_t<<<1, 1, 0, c->stream>>>(c->t_dev, (uint32_t)c->t);
+            c->launches += 1;
+        }
+        if (cudaGraphLaunch(c->graph[which], c->stream) != cudaSuccess) { cudaGetLastError(); c->graph_off = true; c->t_dev_value = ~0ull; break; }
+        c->t += GRAPH_SWEEPS;
+        c->t_dev_value = c->t;
+        c->launches += 3 * GRAPH_SWEEPS + 1;
+        done += GRAPH_SWEEPS;
+        c->last_algo = c->algo;
+        c->have_labels = true;
+    }
+    return done;
+}
 
 int one_sweep(sw_ctx *c, cudaEvent_t *ev = nullptr, unsigned long long *obs_row = nullptr)
 {
@@ -330,6 +389,8 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
     c->table = (uint32_t *)(c->ws + c->cv.table);
     c->obs = (unsigned long long *)(c->ws + c->cv.obs);
     c->flag = (int *)(c->ws + c->cv.flag);
+    c->t_dev = (uint32_t *)(c->ws + c->cv.flag + 32);     // second half of the flag slot
+    if (const char *ng = std::getenv("SW_NO_GRAPH")) c->graph_off = std::atoi(ng) != 0;
     c->stats = (unsigned long long *)(c->ws + c->cv.stats);
     c->ring = (unsigned long long *)(c->ws + c->cv.ring);
     c->tiled_ws = c->ws + c->cv.tiled;
@@ -401,6 +462,7 @@ void sw_destroy(sw_ctx *c)
     DeviceGuard guard(c);
     if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
     if (c->rec_host) cudaFreeHost(c->rec_host);
+    for (int k = 0; k < 2; ++k) if (c->graph[k]) cudaGraphExecDestroy(c->graph[k]);
     if (c->own_ws && c->ws) cudaFree(c->ws);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
     delete c;
@@ -420,6 +482,7 @@ int sw_sweep_async(sw_ctx *c, int n)
         c->t += (uint64_t)n;
         n = 0;
     }
+    if (c->algo == SW_ALGO_TILED && !c->stats_on) n -= graph_sweeps(c, n);
     for (int k = 0; k < n; ++k) {
         int rc = one_sweep(c);
         if (rc != SW_OK) return rc;

@@ -247,7 +247,7 @@ template <int MODEL, bool OBS, bool BATCH>
 __global__ void __launch_bounds__(TILE_THREADS, BATCH ? 4 : SW_LABEL_MINB)
 k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, const __grid_constant__ CUtensorMap spin_map,
              uint16_t *lab16, unsigned long long *parent, uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount,
-             int fuse, unsigned long long *stats, unsigned long long *obs, BatchView bv)
+             int fuse, unsigned long long *stats, unsigned long long *obs, BatchView bv, const uint32_t *t_dev)
 {
     // OBS (q = 2 Potts only, "+ measurement" of PAPER.md:75): S5 fused into phase A.  With two states the
     // XOR of a spin word with its +x / +y neighbour word has byte 1 exactly on the unequal bonds, so three POPC per four
@@ -272,6 +272,7 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
 
     if (threadIdx.x == 0u) mbar_init(&s_bar, 1u);
     pdl_prologue();
+    if (t_dev) t += __ldcg(t_dev);     // launches replayed from a CUDA graph: t = offset inside the graph + the device-side sweep counter
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t tiles_x = L / TW;
@@ -857,7 +858,7 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
 template <int MODEL, bool BATCH>
 __global__ void __launch_bounds__(TILE_THREADS, SW_FLIP_MINB)
 k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsigned long long *parent, const uint32_t *ocount,
-            const uint8_t *in, uint8_t *out, BatchView bv)
+            const uint8_t *in, uint8_t *out, BatchView bv, const uint32_t *t_dev)
 {
     constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
     __shared__ uint8_t s_dec[OCAP + NDEC];   // [pos] decision of the tile's open root pos; [DEC_BASE + d] = d
@@ -870,6 +871,7 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsi
     const uint32_t tx = ltile % tiles_x, ty = ltile / tiles_x;
     const uint32_t x0 = tx * TW, y0 = ty * TH;
     pdl_prologue();   // before every global load, also those of the constant per-lattice keys (tests/test_abi.py reads the SASS)
+    if (t_dev) t += __ldcg(t_dev);     // CUDA-graph replay: see k_tile_label
     PhiloxKey key_lat;
     if (BATCH) {
         key_lat = bv.keys[lat];
@@ -950,6 +952,14 @@ __global__ void k_resolve_labels(Model md, const uint16_t *lab16, const unsigned
     else out[j] = (int32_t)root_site(v, x - x % TW, y - y % TH, L);
 }
 
+// Last node of a captured chunk of sweeps: the device-side sweep counter moves on by the chunk's length.
+__global__ void k_advance_t(uint32_t *t_dev, uint32_t by)
+{
+    pdl_prologue();
+    if (threadIdx.x == 0u && blockIdx.x == 0u) *t_dev += by;
+}
+__global__ void k_set_t(uint32_t *t_dev, uint32_t value) { *t_dev = value; }
+
 // ---------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------
@@ -1020,7 +1030,7 @@ static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k
 // thresholds inside `md` are then unused).
 static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
                                       unsigned long long *parent, int fuse, cudaStream_t stream, unsigned long long *stats,
-                                      unsigned long long *obs = nullptr)
+                                      unsigned long long *obs = nullptr, const uint32_t *t_dev = nullptr)
 {
     const uint32_t tiles = ((uint32_t)md.L / TW) * ((uint32_t)md.L / TH) * st.nlat;
     if (g_pdl_dynamic_smem) {      // occupancy experiments only
@@ -1034,18 +1044,18 @@ static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, co
     if (st.batch) {
         if (md.model == 0)
             return launch_pdl(k_tile_label<0, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
-                              st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+                              st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
         return launch_pdl(k_tile_label<1, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
-                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
     }
     if (md.model == 0 && md.q == 2 && obs)
         return launch_pdl(k_tile_label<0, true, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
-                          st.vedge, st.edges, st.ocount, fuse, stats, obs, st.bv);
+                          st.vedge, st.edges, st.ocount, fuse, stats, obs, st.bv, t_dev);
     if (md.model == 0)
         return launch_pdl(k_tile_label<0, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
-                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
     return launch_pdl(k_tile_label<1, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
-                      st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+                      st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
 }
 
 static inline cudaError_t tiled_launch_merge(TiledState &st, const Model &md, unsigned long long *parent, cudaStream_t stream,
@@ -1064,23 +1074,23 @@ static inline bool tiled_fuses_observables(const Model &md) { return md.model ==
 
 static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
                               uint8_t *out, unsigned long long *parent, cudaStream_t stream, unsigned long long *stats,
-                              uint64_t *launches, cudaEvent_t *ev, unsigned long long *obs = nullptr)
+                              uint64_t *launches, cudaEvent_t *ev, unsigned long long *obs = nullptr, const uint32_t *t_dev = nullptr)
 {
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tiles = (L / TW) * (L / TH) * st.nlat;
     if (ev) cudaEventRecord(ev[0], stream);
-    cudaError_t e = tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats, obs);
+    cudaError_t e = tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats, obs, t_dev);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[1], stream);
     e = tiled_launch_merge(st, md, parent, stream, stats);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[2], stream);
     if (st.batch)
-        e = md.model == 0 ? launch_pdl(k_tile_flip<0, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv)
-                          : launch_pdl(k_tile_flip<1, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv);
+        e = md.model == 0 ? launch_pdl(k_tile_flip<0, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv, t_dev)
+                          : launch_pdl(k_tile_flip<1, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv, t_dev);
     else
-        e = md.model == 0 ? launch_pdl(k_tile_flip<0, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv)
-                          : launch_pdl(k_tile_flip<1, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv);
+        e = md.model == 0 ? launch_pdl(k_tile_flip<0, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv, t_dev)
+                          : launch_pdl(k_tile_flip<1, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv, t_dev);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[3], stream);
     *launches += 3;
