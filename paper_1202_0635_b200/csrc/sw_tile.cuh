@@ -91,6 +91,19 @@ constexpr int NDEC = 16;               // decisions are < q <= 16
 constexpr int DEC_BASE = 512;           // lab16 value DEC_BASE + d: "closed cluster, decision d" (= OCAP)
 constexpr int ECNT = 2 * TH + 2 * TW;     // edge labels exported per tile: left column, right column, top row, bottom row
 constexpr int OCAP = 512;               // open roots listed per tile (<= 128 + 64 + 128 + 64 boundary positions)
+// Output value of a site: DEC_BASE + d (closed cluster, decision d < 16) or LOPEN | (POS_BASE + pos) (open cluster, node pos
+// of its tile).  POS_BASE = 16 makes the LOW BYTE of the value a complete code whenever the tile has at most NARROW_MAX
+// open roots (closed: d < 16, open: 16 + pos <= 255): such a tile ("narrow", almost every tile) writes one byte per site to
+// lab8 instead of two to lab16, which halves the label traffic of K1 and K3.  A tile with more open roots, and the label
+// export (fuse = 0: the values are 14-bit tile-local indices), use lab16; bit 31 of ocount[tile] says which.
+constexpr uint32_t POS_BASE = 16u;
+#ifndef SW_NARROW_MAX
+#define SW_NARROW_MAX 239   // tests build a variant with a small value to mix both formats
+#endif
+constexpr uint32_t NARROW_MAX = SW_NARROW_MAX;
+constexpr uint32_t WIDE_FLAG = 0x80000000u;
+static_assert(NARROW_MAX + POS_BASE <= 255u, "narrow code must fit a byte");
+static_assert(2 * (TW + TH) + POS_BASE <= DEC_BASE, "open codes must stay below the closed ones");
 static_assert(LAB_WORDS <= (int)LMASK + 1, "skewed local index must fit the label field");
 static_assert((TILE_THREADS / 32) * ROWS_PER_WARP == TH, "phase A row split");
 
@@ -105,7 +118,8 @@ struct BatchView {
 };
 
 struct TiledState {
-    uint16_t *lab16 = nullptr;   // [L][L] tile-local root of every site (+ LOPEN)
+    uint16_t *lab16 = nullptr;   // [L][L] output value of every site of a wide tile (or tile-local root, label export)
+    uint8_t *lab8 = nullptr;     // [L][L] low byte of the output value of every site of a narrow tile
     uint32_t *hedge = nullptr;   // [L/128][L/32]  bit (y & 31) of word y >> 5: +x bond of column 128 tx + 127, row y
     uint32_t *vedge = nullptr;   // [L/TH][L/32]   bit (x & 31) of word x >> 5: +y bond of row TH ty + TH - 1, column x
     uint16_t *edges = nullptr;   // [tiles][ECNT]  lab16 values of the tile's boundary sites: left col, right col, top row, bottom row
@@ -246,7 +260,7 @@ __global__ void k_selftest_compare(const uint32_t *vals, int n, int *bad)
 template <int MODEL, bool OBS, bool BATCH>
 __global__ void __launch_bounds__(TILE_THREADS, BATCH ? 4 : SW_LABEL_MINB)
 k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, const __grid_constant__ CUtensorMap spin_map,
-             uint16_t *lab16, unsigned long long *parent, uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount,
+             uint16_t *lab16, uint8_t *lab8, unsigned long long *parent, uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount,
              int fuse, unsigned long long *stats, unsigned long long *obs, BatchView bv, const uint32_t *t_dev)
 {
     // OBS (q = 2 Potts only, "+ measurement" of PAPER.md:75): S5 fused into phase A.  With two states the
@@ -288,6 +302,7 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         md.table = bv.tables + (size_t)lat * (2 * 16) * (2 * 16);
         spins += (size_t)lat * md.N;
         lab16 += (size_t)lat * md.N;
+        lab8 += (size_t)lat * md.N;
         hedge += (size_t)lat * tiles_x * (L / 32);
         vedge += (size_t)lat * (L / TH) * (L / 32);
     }
@@ -580,7 +595,7 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
                     const uint32_t pos = atomicAdd(&s_nopen, 1u);
                     const uint32_t node = blockIdx.x * (uint32_t)OCAP + pos;
                     parent[node] = ((unsigned long long)root_site(a >> 2, x0, y0, L) << 32) | node;
-                    atomicOr(reinterpret_cast<uint32_t *>(lab + a), pos << 16);
+                    atomicOr(reinterpret_cast<uint32_t *>(lab + a), (POS_BASE + pos) << 16);
                 }
             }
         }
@@ -650,7 +665,6 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
     }
     __syncthreads();
     {
-        if (tid == 0u) ocount[blockIdx.x] = s_nopen;
         auto decide = [&](uint32_t o) {           // o = offset of the entry of a closed root
             const uint32_t sp = o >> 2;
             uint32_t out = sp;
@@ -711,29 +725,49 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
     __syncwarp();
     SW_PHASE(5)
 
-    // B4b: per-site labels of the word (64 contiguous bytes)
+    // B4b: per-site labels of the word: 32 contiguous bytes (narrow tile) or 64 (wide tile, label export)
     {
+        const uint32_t nopen = s_nopen;
+        const bool narrow = fuse && nopen <= NARROW_MAX;
+        if (tid == 0u) ocount[blockIdx.x] = nopen | (narrow ? 0u : WIDE_FLAG);
         uint32_t xs[32];
 #pragma unroll
         for (int k = 0; k < 32; ++k) xs[k] = ((S >> k) & 1u) ? lab_ld(lab, sb + 4u * k) : 0u;
-        uint32_t cur = 0u, o[16];
+        uint16_t *ed = edges + (size_t)blockIdx.x * ECNT;       // the labels of the tile's boundary sites, compact, for K2
+        const bool edge_row = wy == 0u || wy == (uint32_t)TH - 1u;
+        uint32_t cur = 0u;
+        if (narrow) {
+            uint32_t o8[8];
 #pragma unroll
-        for (int k = 0; k < 32; ++k) {
-            if ((S >> k) & 1u) cur = xs[k];          // upper half = output value of the run's root (B3b)
-            if (k & 1) o[k >> 1] |= cur & 0xFFFF0000u; else o[k >> 1] = cur >> 16;
+            for (int k = 0; k < 32; ++k) {
+                if ((S >> k) & 1u) cur = xs[k];      // upper half = output value of the run's root (B3, B3b); byte 2 = its low byte
+                o8[k >> 2] = (k & 3) == 0 ? (cur >> 16) & 0xFFu : __byte_perm(o8[k >> 2], cur, (k & 3) == 1 ? 0x3260 : (k & 3) == 2 ? 0x3610 : 0x6210);
+            }
+            uint4 *dst = reinterpret_cast<uint4 *>(lab8 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
+            dst[0] = make_uint4(o8[0], o8[1], o8[2], o8[3]);
+            dst[1] = make_uint4(o8[4], o8[5], o8[6], o8[7]);
         }
-        uint4 *dst = reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
+        if (!narrow || edge_row) {
+            uint32_t o[16];
+            cur = 0u;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) dst[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
-        // the labels of the tile's boundary sites, compact, for K2
-        uint16_t *ed = edges + (size_t)blockIdx.x * ECNT;
-        if (ww == 0u) ed[wy] = (uint16_t)o[0];
-        if (ww == (uint32_t)NWORD - 1u) ed[TH + wy] = (uint16_t)(o[15] >> 16);
-        if (wy == 0u || wy == (uint32_t)TH - 1u) {
-            uint4 *de = reinterpret_cast<uint4 *>(ed + 2 * TH + (wy ? TW : 0) + ww * 32u);
+            for (int k = 0; k < 32; ++k) {
+                if ((S >> k) & 1u) cur = xs[k];
+                if (k & 1) o[k >> 1] |= cur & 0xFFFF0000u; else o[k >> 1] = cur >> 16;
+            }
+            if (!narrow) {
+                uint4 *dst = reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
 #pragma unroll
-            for (int c = 0; c < 4; ++c) de[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
+                for (int c = 0; c < 4; ++c) dst[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
+            }
+            if (edge_row) {
+                uint4 *de = reinterpret_cast<uint4 *>(ed + 2 * TH + (wy ? TW : 0) + ww * 32u);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) de[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
+            }
         }
+        if (ww == 0u) ed[wy] = (uint16_t)(xs[0] >> 16);                            // bit 0 of S is always set
+        if (ww == (uint32_t)NWORD - 1u) ed[TH + wy] = (uint16_t)(cur >> 16);       // the last run's value
         SW_PHASE(6)
         if (stats) {
             const uint32_t n2 = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popc(S));
@@ -848,7 +882,7 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
     const uint32_t same = __match_any_sync(act, pair);
     if ((uint32_t)__ffs((int)same) - 1u != (threadIdx.x & 31u)) return;
     if (stats) atomicAdd(stats + 1, 1ull);
-    gunion(parent, ta * OCAP + (a & (OCAP - 1u)), tb * OCAP + (b & (OCAP - 1u)));
+    gunion(parent, ta * OCAP + ((a & 0x3FFu) - POS_BASE), tb * OCAP + ((b & 0x3FFu) - POS_BASE));
 }
 
 // K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).  in = S^t, out = S^{t+1}.
@@ -857,11 +891,13 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
 #endif
 template <int MODEL, bool BATCH>
 __global__ void __launch_bounds__(TILE_THREADS, SW_FLIP_MINB)
-k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsigned long long *parent, const uint32_t *ocount,
+k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, const uint8_t *lab8, unsigned long long *parent, const uint32_t *ocount,
             const uint8_t *in, uint8_t *out, BatchView bv, const uint32_t *t_dev)
 {
     constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
-    __shared__ uint8_t s_dec[OCAP + NDEC];   // [pos] decision of the tile's open root pos; [DEC_BASE + d] = d
+    // decision table, indexed by the low 10 bits of a site's output value (wide tile) or by its low byte (narrow tile):
+    // [d] = [DEC_BASE + d] = d for the closed clusters, [POS_BASE + pos] = decision of the tile's open root pos
+    __shared__ uint8_t s_dec[DEC_BASE + NDEC];
 
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tid = threadIdx.x;
@@ -876,6 +912,7 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsi
     if (BATCH) {
         key_lat = bv.keys[lat];
         lab16 += (size_t)lat * md.N;
+        lab8 += (size_t)lat * md.N;
         in += (size_t)lat * md.N;
         out += (size_t)lat * md.N;
     }
@@ -883,22 +920,30 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsi
 
     // one decision per open root of the tile (S3; R5 CLUSTER stream), keyed on the site index of the root
     // of its cluster in the global union-find
-    const uint32_t no = ocount[blockIdx.x];
+    const uint32_t oc = ocount[blockIdx.x];
+    const uint32_t no = oc & ~WIDE_FLAG;
+    const bool wide = (oc & WIDE_FLAG) != 0u;        // the tile's labels are in lab16 (two bytes per site), else in lab8
     uint32_t r = 0u;
     if (tid < no) r = groot_site_compress(parent, blockIdx.x * (uint32_t)OCAP + tid);
-    uint4 lab[PASSES];
+    uint4 lab[PASSES];                               // narrow: .x, .y hold the 8 bytes of 8 sites
 #pragma unroll
     for (int c = 0; c < PASSES; ++c) {
         const uint32_t p8 = ((uint32_t)c * TILE_THREADS + tid) * 8u;
-        lab[c] = *reinterpret_cast<const uint4 *>(lab16 + (size_t)(y0 + p8 / TW) * L + x0 + p8 % TW);
+        const size_t at = (size_t)(y0 + p8 / TW) * L + x0 + p8 % TW;
+        if (wide) {
+            lab[c] = *reinterpret_cast<const uint4 *>(lab16 + at);
+        } else {
+            const uint2 b8 = *reinterpret_cast<const uint2 *>(lab8 + at);
+            lab[c] = make_uint4(b8.x, b8.y, 0u, 0u);
+        }
     }
-    if (tid < (uint32_t)NDEC) s_dec[DEC_BASE + tid] = (uint8_t)tid;
+    if (tid < (uint32_t)NDEC) { s_dec[DEC_BASE + tid] = (uint8_t)tid; s_dec[tid] = (uint8_t)tid; }
     for (uint32_t i = tid; i < no; i += TILE_THREADS) {
         if (i >= TILE_THREADS) r = groot_site_compress(parent, blockIdx.x * (uint32_t)OCAP + i);
         uint32_t w[4];
         philox_stream<STREAM_CLUSTER>(key, r >> 2, t, w);
         const uint32_t ww = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
-        s_dec[i] = (uint8_t)(MODEL == 0 ? mulhi_q(ww, (uint32_t)md.q) : (ww >> 31));
+        s_dec[POS_BASE + i] = (uint8_t)(MODEL == 0 ? mulhi_q(ww, (uint32_t)md.q) : (ww >> 31));
     }
     __syncthreads();
 
@@ -911,8 +956,13 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsi
         const size_t at = (size_t)(y0 + p8 / TW) * L + x0 + p8 % TW;
         const uint32_t w[4] = { lab[c].x, lab[c].y, lab[c].z, lab[c].w };
         uint32_t d[8];
+        if (wide) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) d[j] = s_dec[(w[j >> 1] >> (16 * (j & 1))) & 0x3FFu];   // LOPEN | pos or DEC_BASE + d
+            for (int j = 0; j < 8; ++j) d[j] = s_dec[(w[j >> 1] >> (16 * (j & 1))) & 0x3FFu];   // LOPEN | POS_BASE + pos or DEC_BASE + d
+        } else {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) d[j] = s_dec[(w[j >> 2] >> (8 * (j & 3))) & 0xFFu];     // POS_BASE + pos or d
+        }
         uint2 o;
         if (MODEL == 0) {
             o.x = d[0] | (d[1] << 8) | (d[2] << 16) | (d[3] << 24);
@@ -920,17 +970,17 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, unsi
         } else {
             const uint2 old = *reinterpret_cast<const uint2 *>(in + at);
             const uint32_t q = (uint32_t)md.q;
-            uint32_t s[8];
+            uint32_t sp[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                s[j] = (((j < 4) ? old.x : old.y) >> (8 * (j & 3))) & 0xFFu;
+                sp[j] = (((j < 4) ? old.x : old.y) >> (8 * (j & 3))) & 0xFFu;
                 if (d[j]) {
-                    const uint32_t vv = m + q - s[j];          // in (0, 2q)
-                    s[j] = vv >= q ? vv - q : vv;
+                    const uint32_t vv = m + q - sp[j];          // in (0, 2q)
+                    sp[j] = vv >= q ? vv - q : vv;
                 }
             }
-            o.x = s[0] | (s[1] << 8) | (s[2] << 16) | (s[3] << 24);
-            o.y = s[4] | (s[5] << 8) | (s[6] << 16) | (s[7] << 24);
+            o.x = sp[0] | (sp[1] << 8) | (sp[2] << 16) | (sp[3] << 24);
+            o.y = sp[4] | (sp[5] << 8) | (sp[6] << 16) | (sp[7] << 24);
         }
         *reinterpret_cast<uint2 *>(out + at) = o;
     }
@@ -948,7 +998,7 @@ __global__ void k_resolve_labels(Model md, const uint16_t *lab16, const unsigned
     const uint32_t y = i / L, x = i - y * L;
     const uint32_t v = lab16[i];
     // written with fuse = 0: closed -> tile-local root sp; open -> LOPEN | pos
-    if (v & LOPEN) out[j] = (int32_t)groot_site(parent, ((y / TH) * (L / TW) + x / TW) * (uint32_t)OCAP + (v & (OCAP - 1u)));
+    if (v & LOPEN) out[j] = (int32_t)groot_site(parent, ((y / TH) * (L / TW) + x / TW) * (uint32_t)OCAP + ((v & 0x3FFu) - POS_BASE));
     else out[j] = (int32_t)root_site(v, x - x % TW, y - y % TH, L);
 }
 
@@ -996,7 +1046,7 @@ static inline size_t tiled_workspace_bytes_n(int L, size_t nlat)
     if (!tiled_supported(L)) return 0;
     const size_t N = (size_t)L * L;
     const size_t tiles = (size_t)(L / TW) * (L / TH);
-    return nlat * 2 * N + 1024 + nlat * (size_t)(L / TW) * (L / 32) * 4 + 1024 + nlat * (size_t)(L / TH) * (L / 32) * 4 + 1024 +
+    return nlat * 2 * N + 1024 + nlat * N + 1024 + nlat * (size_t)(L / TW) * (L / 32) * 4 + 1024 + nlat * (size_t)(L / TH) * (L / 32) * 4 + 1024 +
            nlat * tiles * ECNT * 2 + 1024 + nlat * tiles * 4 + 1024;
 }
 
@@ -1011,6 +1061,8 @@ static inline int tiled_init(TiledState &st, const Model &md, char *ws, const ui
     size_t off = 0;
     st.lab16 = reinterpret_cast<uint16_t *>(ws);
     off += (nlat * 2 * L * L + 1023) / 1024 * 1024;
+    st.lab8 = reinterpret_cast<uint8_t *>(ws + off);
+    off += (nlat * L * L + 1023) / 1024 * 1024;
     st.hedge = reinterpret_cast<uint32_t *>(ws + off);
     off += (nlat * (L / TW) * (L / 32) * 4 + 1023) / 1024 * 1024;
     st.vedge = reinterpret_cast<uint32_t *>(ws + off);
@@ -1043,18 +1095,18 @@ static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, co
     unsigned long long *const none = nullptr;
     if (st.batch) {
         if (md.model == 0)
-            return launch_pdl(k_tile_label<0, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+            return launch_pdl(k_tile_label<0, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
                               st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
-        return launch_pdl(k_tile_label<1, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+        return launch_pdl(k_tile_label<1, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
                           st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
     }
     if (md.model == 0 && md.q == 2 && obs)
-        return launch_pdl(k_tile_label<0, true, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+        return launch_pdl(k_tile_label<0, true, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
                           st.vedge, st.edges, st.ocount, fuse, stats, obs, st.bv, t_dev);
     if (md.model == 0)
-        return launch_pdl(k_tile_label<0, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+        return launch_pdl(k_tile_label<0, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
                           st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
-    return launch_pdl(k_tile_label<1, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, parent, st.hedge,
+    return launch_pdl(k_tile_label<1, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
                       st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
 }
 
@@ -1086,11 +1138,11 @@ static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[2], stream);
     if (st.batch)
-        e = md.model == 0 ? launch_pdl(k_tile_flip<0, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv, t_dev)
-                          : launch_pdl(k_tile_flip<1, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv, t_dev);
+        e = md.model == 0 ? launch_pdl(k_tile_flip<0, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv, t_dev)
+                          : launch_pdl(k_tile_flip<1, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv, t_dev);
     else
-        e = md.model == 0 ? launch_pdl(k_tile_flip<0, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv, t_dev)
-                          : launch_pdl(k_tile_flip<1, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, parent, st.ocount, in, out, st.bv, t_dev);
+        e = md.model == 0 ? launch_pdl(k_tile_flip<0, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv, t_dev)
+                          : launch_pdl(k_tile_flip<1, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv, t_dev);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[3], stream);
     *launches += 3;

@@ -1,6 +1,6 @@
 """The overflow paths of the tile kernel (union-edge list, root list) are unreachable with the production list
 capacities on the paper's workloads; this test builds the same library with tiny capacities (SW_EDGE_CAP=8,
-SW_RCAP=16) so that every warp overflows both lists, and checks parity with the oracle, bit for bit."""
+SW_RCAP=16, SW_NARROW_MAX=40: tiles with more open roots write two bytes per site) so that every warp overflows both lists and both label formats occur, and checks parity with the oracle, bit for bit."""
 import os
 import subprocess
 import sys
@@ -36,7 +36,7 @@ def test_tiny_list_capacities_match_the_oracle(tmp_path):
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
     from paper_1202_0635_b200 import build
     lib = tmp_path / "libsw_tiny.so"
-    cmd = [os.environ.get("NVCC", "nvcc"), *build.NVCC_FLAGS, "-DSW_EDGE_CAP=8", "-DSW_RCAP=16",
+    cmd = [os.environ.get("NVCC", "nvcc"), *build.NVCC_FLAGS, "-DSW_EDGE_CAP=8", "-DSW_RCAP=16", "-DSW_NARROW_MAX=40",
            "-I", str(ROOT / "include"), "-I", str(build.CSRC), "-o", str(lib)] + [str(s) for s in build.sources()]
     subprocess.run(cmd, check=True)
     env = dict(os.environ, SW_LIB=str(lib))
