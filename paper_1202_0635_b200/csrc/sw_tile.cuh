@@ -15,17 +15,19 @@
 //                 tile-wide and every thread draws one cluster decision per round (CLUSTER stream keyed on the root's
 //                 global site index); B4: every run resolves to its root.  Labels in shared memory are byte offsets
 //                 (a pointer hop is one LDS), the pointer in the low half of an entry, the output value in the high half.
-//        output   one uint16 per site: DEC_BASE + decision (closed cluster) or LOPEN | pos (open cluster); the labels
+//        output   one byte per site: decision (closed cluster) or 16 + pos (open cluster) -- the low byte of the 16-bit
+//                 value DEC_BASE + decision / LOPEN | 16 + pos that tiles with many open roots write instead; the labels
 //                 of the tile's boundary sites also go to a compact edge array for K2.
 //   K2 k_seam_merge   S2b: union across every active tile-crossing bond in the global union-find over open roots
 //                     (64-bit keys (site index, node), atomicMin: the root of a cluster is its minimum site index).
 //   K3 k_tile_flip    S3 for open clusters + S4.  Per tile: one decision per open root, keyed on the site index of its
-//                     global root; then every site looks its 16-bit label up in a 528-byte table and the new spin is
+//                     global root; then every site looks its label up in a 528-byte table and the new spin is
 //                     written to the other ping-pong buffer.
 //
 // The root of a cluster is its minimum site index at both levels (row-major order inside a tile equals the order
 // of the global indices), so spins, labels and observables equal the oracle's bit for bit.
-// HBM traffic per site and sweep: K1 1 B (spins) + 2 B (labels); K3 2 B (labels) [+ 1 B spins, clock] + 1 B.
+// HBM traffic per site and sweep: K1 1 B (spins) + 1 B (labels: 2 B for a tile with more than NARROW_MAX open roots);
+// K3 1 B (labels) [+ 1 B spins, clock] + 1 B.
 #pragma once
 #include <cuda.h>            // CUtensorMap (types only: the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
