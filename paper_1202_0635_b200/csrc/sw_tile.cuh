@@ -182,9 +182,8 @@ __device__ __forceinline__ void sunion(char *lab, uint32_t a, uint32_t b)
     }
 }
 
-// Two A/B switches kept for the record (both measured slower on B200): SW_K1_HILO = mask of the
-// Philox rounds of the labeling kernel computed as IMAD.HI + IMAD (sw_philox.cuh); SW_CLZ_LOOPS = loops over the set
-// bits of a mask take the highest bit first (one FLO per step instead of BREV + FLO).
+// An A/B switch kept for the record (measured slower on B200): SW_K1_HILO = mask of the Philox
+// rounds of the labeling kernel computed as IMAD.HI + IMAD (sw_philox.cuh).
 #ifndef SW_K1_HILO
 #define SW_K1_HILO 0u
 #endif
@@ -197,13 +196,9 @@ __device__ __forceinline__ uint32_t top_bit(uint32_t x)
 }
 __device__ __forceinline__ uint32_t pop_top(uint32_t &c)
 {
-#ifndef SW_CLZ_LOOPS
-    const uint32_t k = (uint32_t)__ffs((int)c) - 1u;
-    c &= c - 1u;
-#else
+    // highest bit first: one FLO (bfind); lowest first (__ffs) is BREV + FLO, two trips through the slow XU pipe
     const uint32_t k = top_bit(c);
     c ^= 1u << k;
-#endif
     return k;
 }
 
@@ -748,28 +743,34 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
             uint4 *dst = reinterpret_cast<uint4 *>(lab8 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
             dst[0] = make_uint4(o8[0], o8[1], o8[2], o8[3]);
             dst[1] = make_uint4(o8[4], o8[5], o8[6], o8[7]);
-        }
-        if (!narrow || edge_row) {
+            if (edge_row) {                          // K2 reads 16-bit entries: the bytes, zero-extended (it uses the low 10 bits)
+                uint4 *de = reinterpret_cast<uint4 *>(ed + 2 * TH + (wy ? TW : 0) + ww * 32u);
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+                    de[c] = make_uint4(__byte_perm(o8[2 * c], 0u, 0x4140), __byte_perm(o8[2 * c], 0u, 0x4342),
+                                       __byte_perm(o8[2 * c + 1], 0u, 0x4140), __byte_perm(o8[2 * c + 1], 0u, 0x4342));
+            }
+        } else {
             uint32_t o[16];
-            cur = 0u;
 #pragma unroll
             for (int k = 0; k < 32; ++k) {
                 if ((S >> k) & 1u) cur = xs[k];
                 if (k & 1) o[k >> 1] |= cur & 0xFFFF0000u; else o[k >> 1] = cur >> 16;
             }
-            if (!narrow) {
-                uint4 *dst = reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
+            uint4 *dst = reinterpret_cast<uint4 *>(lab16 + (size_t)(y0 + wy) * L + x0 + ww * 32u);
 #pragma unroll
-                for (int c = 0; c < 4; ++c) dst[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
-            }
+            for (int c = 0; c < 4; ++c) dst[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
             if (edge_row) {
                 uint4 *de = reinterpret_cast<uint4 *>(ed + 2 * TH + (wy ? TW : 0) + ww * 32u);
 #pragma unroll
                 for (int c = 0; c < 4; ++c) de[c] = make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]);
             }
         }
-        if (ww == 0u) ed[wy] = (uint16_t)(xs[0] >> 16);                            // bit 0 of S is always set
-        if (ww == (uint32_t)NWORD - 1u) ed[TH + wy] = (uint16_t)(cur >> 16);       // the last run's value
+        // left / right column: the first and the last run's value (bit 0 of S is always set); a narrow tile exports the
+        // low byte only, like its rows
+        const uint32_t emask = narrow ? 0xFFu : 0xFFFFu;
+        if (ww == 0u) ed[wy] = (uint16_t)((xs[0] >> 16) & emask);
+        if (ww == (uint32_t)NWORD - 1u) ed[TH + wy] = (uint16_t)((cur >> 16) & emask);
         SW_PHASE(6)
         if (stats) {
             const uint32_t n2 = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popc(S));
