@@ -363,16 +363,19 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
                 if (j < ROWS_PER_WARP) hal[j] = clock_c4(hal[j], m, q2) & 0xFFu;
             }
         }
+        const uint32_t pair0 = ((y0 + ly0) * L + gx) >> 1;           // (L and gx are multiples of 4)
+        const bool writer = (lane & 7u) == 0u;                        // the lane that holds the gathered word of 32 sites
+        uint32_t *const hrow = &s_H[ly0][lane >> 3], *const vrow = &s_V[ly0][lane >> 3];
 #pragma unroll
         for (int j = 0; j < ROWS_PER_WARP; ++j) {
             const uint32_t cur = row[j], nxt = row[j + 1];
             uint32_t rn = __shfl_down_sync(0xFFFFFFFFu, cur, 1) & 0xFFu;
             if (lane == 31u) rn = hal[j];
             const uint32_t right = (cur >> 8) | (rn << 24);       // byte k = +x neighbour of site k
-            const uint32_t i0 = (y0 + ly0 + j) * L + gx;
+            const uint32_t c0 = pair0 + (uint32_t)j * (L >> 1);     // counter of the first of this lane's two site pairs in row j
             uint32_t wa[4], wb[4];
-            philox_stream<STREAM_BOND, SW_K1_HILO>(key, i0 >> 1, t, wa);
-            philox_stream<STREAM_BOND, SW_K1_HILO>(key, (i0 >> 1) + 1u, t, wb);
+            philox_stream<STREAM_BOND, SW_K1_HILO>(key, c0, t, wa);
+            philox_stream<STREAM_BOND, SW_K1_HILO>(key, c0 + 1u, t, wb);
             uint32_t hn = 0u, vn = 0u;
             if (MODEL == 0) {
                 // [w >= th] is the carry of w + (2^32 - th); add-with-carry shifts it into a nibble (two ALU instructions
@@ -403,9 +406,9 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
             c |= __shfl_down_sync(0xFFFFFFFFu, c, 1) << 4;
             c |= __shfl_down_sync(0xFFFFFFFFu, c, 2) << 8;
             const uint32_t c4 = __shfl_down_sync(0xFFFFFFFFu, c, 4);
-            if ((lane & 7u) == 0u) {
-                s_H[ly0 + j][lane >> 3] = (c & 0xFFFFu) | (c4 << 16);
-                s_V[ly0 + j][lane >> 3] = (c >> 16) | (c4 & 0xFFFF0000u);
+            if (writer) {
+                hrow[j * NWORD] = (c & 0xFFFFu) | (c4 << 16);
+                vrow[j * NWORD] = (c >> 16) | (c4 & 0xFFFF0000u);
             }
         }
     }
