@@ -75,7 +75,8 @@ void sw_destroy(sw_ctx *ctx);
  * t .. t+n-1 where t = sw_sweep_index().  sw_sweep(a); sw_sweep(b) == sw_sweep(a+b).
  * sw_sweep returns after the work is complete; sw_sweep_async only enqueues it on the stream.
  * Tiled back-end: whole chunks of 16 sweeps are replayed from a CUDA graph (one cudaGraphLaunch per chunk instead of 48
- * kernel launches; the environment variable SW_NO_GRAPH=1, read by sw_create*, turns that off); the result is the same. */
+ * kernel launches; the environment variable SW_NO_GRAPH=1, read by sw_create*, turns that off); the result is the same,
+ * sw_launch_count counts the replayed kernels, sw_stats out[7] the replays. */
 int sw_sweep(sw_ctx *ctx, int n);
 int sw_sweep_async(sw_ctx *ctx, int n);
 int sw_sync(sw_ctx *ctx);
@@ -144,7 +145,8 @@ int sw_get_algorithm(sw_ctx *ctx); /* the back-end actually in use (never SW_ALG
  * PAPER.md:75), HOST output of SW_NUM_STATS doubles: out[0] = sweeps counted, out[1] = cross-tile merge attempts,
  * out[2] = tile-local nodes (horizontal runs), out[3] = tile-local union edges, out[4] = pointer hops of the
  * tile-local resolve pass, out[5] = scan passes of the paper's labellers (SW_ALGO_HAWICK / SW_ALGO_KALENTEV, always
- * counted) and out[6] = the sweeps they served (out[5] / out[6] is the iteration count PAPER.md:75 quotes), out[7] reserved (0), out[8..15] = SM clock cycles the warps of the tile-labeling
+ * counted) and out[6] = the sweeps they served (out[5] / out[6] is the iteration count PAPER.md:75 quotes), out[7] = chunks of sweeps replayed from
+ * a CUDA graph (always counted), out[8..15] = SM clock cycles the warps of the tile-labeling
  * kernel spent in each of its phases (bonds, setup, run scan, unions, open marking, resolve, output, root decisions;
  * summed over warps).  Counters are only collected after sw_enable_stats(ctx, 1) (they cost atomics and clock reads). */
 #define SW_NUM_STATS 16

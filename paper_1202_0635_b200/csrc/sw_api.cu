@@ -107,11 +107,21 @@ struct sw_ctx {
     uint64_t ccl_iterations = 0, ccl_sweeps = 0;   // SW_ALGO_HAWICK / SW_ALGO_KALENTEV: scan passes and the sweeps they served
     sw::TiledState tiled{};
     unsigned long long *rec_host = nullptr;   // pinned copy of the record ring (sw_sweep_record)
-    // Tiled back-end: chunks of GRAPH_SWEEPS sweeps replayed from a CUDA graph (one per parity of the spin ping-pong);
-    // the kernels of a graph read the sweep index as "offset inside the chunk + *t_dev".
-    cudaGraphExec_t graph[2] = { nullptr, nullptr };
-    uint32_t *t_dev = nullptr;
-    uint64_t t_dev_value = ~0ull;             // what *t_dev holds (~0: unknown)
+    // Tiled back-end: chunks of GRAPH_SWEEPS sweeps replayed from a CUDA graph (one per parity of the spin ping-pong).
+    // The sweep index stays a kernel parameter (a uniform value the compiler keeps in uniform registers): before a
+    // replay the t of the 2 * GRAPH_SWEEPS kernel nodes that take one is set with cudaGraphExecKernelNodeSetParams.
+    struct GraphNode {
+        cudaGraphNode_t node;
+        cudaKernelNodeParams params;      // as captured; kernelParams replaced by `kp`
+        std::vector<void *> kp;           // the node's parameter pointers, entry 2 (t) redirected to `t`
+        uint32_t offset, t;               // sweep inside the chunk; value for the next replay
+    };
+    struct SweepGraph {
+        cudaGraph_t graph = nullptr;      // kept alive: the captured parameter storage belongs to it
+        cudaGraphExec_t exec = nullptr;
+        std::vector<GraphNode> nodes;
+    } graph[2];
+    uint64_t graph_replays = 0;
     bool graph_off = false;                   // SW_NO_GRAPH=1, or capture failed once: plain launches from then on
 };
 
@@ -225,14 +235,15 @@ bool fuses_observables(const sw_ctx *c) { return c->algo == SW_ALGO_TILED && sw:
 
 // sw_sweep(n) of the tiled back-end, n >= GRAPH_SWEEPS: the 3 kernels of GRAPH_SWEEPS consecutive sweeps (with their
 // programmatic-dependent-launch edges) are captured once per ping-pong parity and replayed with one cudaGraphLaunch per
-// chunk ("CUDA graph or persistent kernel" as the host scheduler).  GRAPH_SWEEPS is even, so a chunk leaves
-// the roles of the two spin buffers as it found them.
+// chunk, after the sweep indices of its nodes have been set ("CUDA graph or persistent kernel" as the host
+// scheduler).  GRAPH_SWEEPS is even, so a chunk leaves the roles of the two spin buffers as it found them.
 constexpr int GRAPH_SWEEPS = 16;
 
 bool build_graph(sw_ctx *c, int which)
 {
     // captured on a private stream (the context's may be the legacy default stream, which cannot capture); nothing runs
     // on it: the instantiated graph is launched on the context's stream
+    sw_ctx::SweepGraph &sg = c->graph[which];
     cudaStream_t cap = nullptr;
     if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
     if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); cudaStreamDestroy(cap); return false; }
@@ -240,17 +251,41 @@ bool build_graph(sw_ctx *c, int which)
     uint64_t dummy = 0;
     bool ok = true;
     for (int s = 0; s < GRAPH_SWEEPS && ok; ++s) {
-        ok = sw::tiled_sweep(c->tiled, c->md, c->key, (uint32_t)s, a, b, (unsigned long long *)c->labels, cap, nullptr, &dummy, nullptr,
-                             nullptr, c->t_dev) == 0;
+        ok = sw::tiled_sweep(c->tiled, c->md, c->key, (uint32_t)s, a, b, (unsigned long long *)c->labels, cap, nullptr, &dummy, nullptr) == 0;
         std::swap(a, b);
     }
-    ok = ok && sw::launch_pdl(sw::k_advance_t, 1u, 32u, cap, c->t_dev, (uint32_t)GRAPH_SWEEPS) == cudaSuccess;
-    cudaGraph_t g = nullptr;
-    if (cudaStreamEndCapture(cap, &g) != cudaSuccess || !g) ok = false;
+    if (cudaStreamEndCapture(cap, &sg.graph) != cudaSuccess || !sg.graph) ok = false;
     cudaStreamDestroy(cap);
-    if (ok && cudaGraphInstantiate(&c->graph[which], g, 0) != cudaSuccess) { c->graph[which] = nullptr; ok = false; }
-    if (g) cudaGraphDestroy(g);
-    if (!ok) cudaGetLastError();
+    if (ok && cudaGraphInstantiate(&sg.exec, sg.graph, 0) != cudaSuccess) { sg.exec = nullptr; ok = false; }
+    // the kernel nodes that take the sweep index (parameter 2 of the labeling and of the flip kernel; captured with t = the
+    // sweep's offset inside the chunk, which identifies them)
+    size_t n = 0;
+    if (ok && cudaGraphGetNodes(sg.graph, nullptr, &n) != cudaSuccess) ok = false;
+    std::vector<cudaGraphNode_t> all(n);
+    if (ok && n && cudaGraphGetNodes(sg.graph, all.data(), &n) != cudaSuccess) ok = false;
+    const void *label_fn = c->model == SW_POTTS ? (const void *)sw::k_tile_label<0, false, false> : (const void *)sw::k_tile_label<1, false, false>;
+    const void *flip_fn = c->model == SW_POTTS ? (const void *)sw::k_tile_flip<0, false> : (const void *)sw::k_tile_flip<1, false>;
+    for (size_t k = 0; ok && k < n; ++k) {
+        cudaGraphNodeType type;
+        if (cudaGraphNodeGetType(all[k], &type) != cudaSuccess) { ok = false; break; }
+        if (type != cudaGraphNodeTypeKernel) continue;
+        sw_ctx::GraphNode gn;
+        gn.node = all[k];
+        if (cudaGraphKernelNodeGetParams(all[k], &gn.params) != cudaSuccess) { ok = false; break; }
+        const int np = gn.params.func == label_fn ? 16 : gn.params.func == flip_fn ? 10 : 0;
+        if (np == 0) continue;                        // k_seam_merge takes no sweep index
+        gn.kp.assign(gn.params.kernelParams, gn.params.kernelParams + np);
+        gn.offset = *static_cast<const uint32_t *>(gn.kp[2]);
+        gn.t = gn.offset;
+        sg.nodes.push_back(std::move(gn));
+    }
+    ok = ok && sg.nodes.size() == 2u * GRAPH_SWEEPS;
+    if (!ok) {
+        if (sg.exec) cudaGraphExecDestroy(sg.exec);
+        if (sg.graph) cudaGraphDestroy(sg.graph);
+        sg.exec = nullptr; sg.graph = nullptr; sg.nodes.clear();
+        cudaGetLastError();
+    }
     return ok;
 }
 
@@ -260,15 +295,19 @@ int graph_sweeps(sw_ctx *c, int n)
     int done = 0;
     while (n - done >= GRAPH_SWEEPS && !c->graph_off) {
         const int which = c->spins == c->tiled.map_base[0] ? 0 : 1;
-        if (!c->graph[which] && !build_graph(c, which)) { c->graph_off = true; break; }
-        if (c->t_dev_value != c->t) {
-            sw::k_set_t<<<1, 1, 0, c->stream>>>(c->t_dev, (uint32_t)c->t);
-            c->launches += 1;
+        sw_ctx::SweepGraph &sg = c->graph[which];
+        if (!sg.exec && !build_graph(c, which)) { c->graph_off = true; break; }
+        bool ok = true;
+        for (sw_ctx::GraphNode &gn : sg.nodes) {
+            gn.t = (uint32_t)c->t + gn.offset;
+            gn.kp[2] = &gn.t;
+            gn.params.kernelParams = gn.kp.data();
+            ok = ok && cudaGraphExecKernelNodeSetParams(sg.exec, gn.node, &gn.params) == cudaSuccess;
         }
-        if (cudaGraphLaunch(c->graph[which], c->stream) != cudaSuccess) { cudaGetLastError(); c->graph_off = true; c->t_dev_value = ~0ull; break; }
+        if (!ok || cudaGraphLaunch(sg.exec, c->stream) != cudaSuccess) { cudaGetLastError(); c->graph_off = true; break; }
         c->t += GRAPH_SWEEPS;
-        c->t_dev_value = c->t;
-        c->launches += 3 * GRAPH_SWEEPS + 1;
+        c->launches += 3 * GRAPH_SWEEPS;
+        c->graph_replays += 1;
         done += GRAPH_SWEEPS;
         c->last_algo = c->algo;
         c->have_labels = true;
@@ -389,7 +428,6 @@ sw_ctx *create_impl(int L, int q, int model, double T, uint64_t seed, void *ws, 
     c->table = (uint32_t *)(c->ws + c->cv.table);
     c->obs = (unsigned long long *)(c->ws + c->cv.obs);
     c->flag = (int *)(c->ws + c->cv.flag);
-    c->t_dev = (uint32_t *)(c->ws + c->cv.flag + 32);     // second half of the flag slot
     if (const char *ng = std::getenv("SW_NO_GRAPH")) c->graph_off = std::atoi(ng) != 0;
     c->stats = (unsigned long long *)(c->ws + c->cv.stats);
     c->ring = (unsigned long long *)(c->ws + c->cv.ring);
@@ -462,7 +500,10 @@ void sw_destroy(sw_ctx *c)
     DeviceGuard guard(c);
     if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
     if (c->rec_host) cudaFreeHost(c->rec_host);
-    for (int k = 0; k < 2; ++k) if (c->graph[k]) cudaGraphExecDestroy(c->graph[k]);
+    for (int k = 0; k < 2; ++k) {
+        if (c->graph[k].exec) cudaGraphExecDestroy(c->graph[k].exec);
+        if (c->graph[k].graph) cudaGraphDestroy(c->graph[k].graph);
+    }
     if (c->own_ws && c->ws) cudaFree(c->ws);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
     delete c;
@@ -714,6 +755,7 @@ int sw_stats(sw_ctx *c, double *out4)
     out4[0] = (double)c->stat_sweeps;
     out4[5] = (double)c->ccl_iterations;
     out4[6] = (double)c->ccl_sweeps;
+    out4[7] = (double)c->graph_replays;
     return SW_OK;
 }
 

@@ -258,7 +258,7 @@ template <int MODEL, bool OBS, bool BATCH>
 __global__ void __launch_bounds__(TILE_THREADS, BATCH ? 4 : SW_LABEL_MINB)
 k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, const __grid_constant__ CUtensorMap spin_map,
              uint16_t *lab16, uint8_t *lab8, unsigned long long *parent, uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount,
-             int fuse, unsigned long long *stats, unsigned long long *obs, BatchView bv, const uint32_t *t_dev)
+             int fuse, unsigned long long *stats, unsigned long long *obs, BatchView bv)
 {
     // OBS (q = 2 Potts only, "+ measurement" of PAPER.md:75): S5 fused into phase A.  With two states the
     // XOR of a spin word with its +x / +y neighbour word has byte 1 exactly on the unequal bonds, so three POPC per four
@@ -283,7 +283,6 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
 
     if (threadIdx.x == 0u) mbar_init(&s_bar, 1u);
     pdl_prologue();
-    if (t_dev) t += __ldcg(t_dev);     // launches replayed from a CUDA graph: t = offset inside the graph + the device-side sweep counter
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t tiles_x = L / TW;
@@ -898,7 +897,7 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
 template <int MODEL, bool BATCH>
 __global__ void __launch_bounds__(TILE_THREADS, SW_FLIP_MINB)
 k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, const uint8_t *lab8, unsigned long long *parent, const uint32_t *ocount,
-            const uint8_t *in, uint8_t *out, BatchView bv, const uint32_t *t_dev)
+            const uint8_t *in, uint8_t *out, BatchView bv)
 {
     constexpr int PASSES = TILE_SITES / 8 / TILE_THREADS;   // 4
     // decision table, indexed by the low 10 bits of a site's output value (wide tile) or by its low byte (narrow tile):
@@ -913,7 +912,6 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, cons
     const uint32_t tx = ltile % tiles_x, ty = ltile / tiles_x;
     const uint32_t x0 = tx * TW, y0 = ty * TH;
     pdl_prologue();   // before every global load, also those of the constant per-lattice keys (tests/test_abi.py reads the SASS)
-    if (t_dev) t += __ldcg(t_dev);     // CUDA-graph replay: see k_tile_label
     PhiloxKey key_lat;
     if (BATCH) {
         key_lat = bv.keys[lat];
@@ -932,6 +930,8 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, cons
     uint32_t r = 0u;
     if (tid < no) r = groot_site_compress(parent, blockIdx.x * (uint32_t)OCAP + tid);
     uint4 lab[PASSES];                               // narrow: .x, .y hold the 8 bytes of 8 sites
+    uint2 old[PASSES];
+    (void)old;
 #pragma unroll
     for (int c = 0; c < PASSES; ++c) {
         const uint32_t p8 = ((uint32_t)c * TILE_THREADS + tid) * 8u;
@@ -942,6 +942,7 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, cons
             const uint2 b8 = *reinterpret_cast<const uint2 *>(lab8 + at);
             lab[c] = make_uint4(b8.x, b8.y, 0u, 0u);
         }
+        if (MODEL == 1) old[c] = *reinterpret_cast<const uint2 *>(in + at);    // S^t (the reflection needs the old spin)
     }
     if (tid < (uint32_t)NDEC) { s_dec[DEC_BASE + tid] = (uint8_t)tid; s_dec[tid] = (uint8_t)tid; }
     for (uint32_t i = tid; i < no; i += TILE_THREADS) {
@@ -974,12 +975,11 @@ k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, cons
             o.x = d[0] | (d[1] << 8) | (d[2] << 16) | (d[3] << 24);
             o.y = d[4] | (d[5] << 8) | (d[6] << 16) | (d[7] << 24);
         } else {
-            const uint2 old = *reinterpret_cast<const uint2 *>(in + at);
             const uint32_t q = (uint32_t)md.q;
             uint32_t sp[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                sp[j] = (((j < 4) ? old.x : old.y) >> (8 * (j & 3))) & 0xFFu;
+                sp[j] = (((j < 4) ? old[c].x : old[c].y) >> (8 * (j & 3))) & 0xFFu;
                 if (d[j]) {
                     const uint32_t vv = m + q - sp[j];          // in (0, 2q)
                     sp[j] = vv >= q ? vv - q : vv;
@@ -1007,14 +1007,6 @@ __global__ void k_resolve_labels(Model md, const uint16_t *lab16, const unsigned
     if (v & LOPEN) out[j] = (int32_t)groot_site(parent, ((y / TH) * (L / TW) + x / TW) * (uint32_t)OCAP + ((v & 0x3FFu) - POS_BASE));
     else out[j] = (int32_t)root_site(v, x - x % TW, y - y % TH, L);
 }
-
-// Last node of a captured chunk of sweeps: the device-side sweep counter moves on by the chunk's length.
-__global__ void k_advance_t(uint32_t *t_dev, uint32_t by)
-{
-    pdl_prologue();
-    if (threadIdx.x == 0u && blockIdx.x == 0u) *t_dev += by;
-}
-__global__ void k_set_t(uint32_t *t_dev, uint32_t value) { *t_dev = value; }
 
 // ---------------------------------------------------------------------------------------------------------
 // host side
@@ -1088,7 +1080,7 @@ static const char *const TILED_KERNELS[TILED_NUM_KERNELS] = { "k_tile_label", "k
 // thresholds inside `md` are then unused).
 static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
                                       unsigned long long *parent, int fuse, cudaStream_t stream, unsigned long long *stats,
-                                      unsigned long long *obs = nullptr, const uint32_t *t_dev = nullptr)
+                                      unsigned long long *obs = nullptr)
 {
     const uint32_t tiles = ((uint32_t)md.L / TW) * ((uint32_t)md.L / TH) * st.nlat;
     if (g_pdl_dynamic_smem) {      // occupancy experiments only
@@ -1102,18 +1094,18 @@ static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, co
     if (st.batch) {
         if (md.model == 0)
             return launch_pdl(k_tile_label<0, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
-                              st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
+                              st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
         return launch_pdl(k_tile_label<1, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
-                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
+                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
     }
     if (md.model == 0 && md.q == 2 && obs)
         return launch_pdl(k_tile_label<0, true, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
-                          st.vedge, st.edges, st.ocount, fuse, stats, obs, st.bv, t_dev);
+                          st.vedge, st.edges, st.ocount, fuse, stats, obs, st.bv);
     if (md.model == 0)
         return launch_pdl(k_tile_label<0, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
-                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
+                          st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
     return launch_pdl(k_tile_label<1, false, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
-                      st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv, t_dev);
+                      st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
 }
 
 static inline cudaError_t tiled_launch_merge(TiledState &st, const Model &md, unsigned long long *parent, cudaStream_t stream,
@@ -1132,23 +1124,23 @@ static inline bool tiled_fuses_observables(const Model &md) { return md.model ==
 
 static inline int tiled_sweep(TiledState &st, const Model &md, const PhiloxKey &key, uint32_t t, const uint8_t *in,
                               uint8_t *out, unsigned long long *parent, cudaStream_t stream, unsigned long long *stats,
-                              uint64_t *launches, cudaEvent_t *ev, unsigned long long *obs = nullptr, const uint32_t *t_dev = nullptr)
+                              uint64_t *launches, cudaEvent_t *ev, unsigned long long *obs = nullptr)
 {
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tiles = (L / TW) * (L / TH) * st.nlat;
     if (ev) cudaEventRecord(ev[0], stream);
-    cudaError_t e = tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats, obs, t_dev);
+    cudaError_t e = tiled_launch_label(st, md, key, t, in, parent, 1, stream, stats, obs);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[1], stream);
     e = tiled_launch_merge(st, md, parent, stream, stats);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[2], stream);
     if (st.batch)
-        e = md.model == 0 ? launch_pdl(k_tile_flip<0, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv, t_dev)
-                          : launch_pdl(k_tile_flip<1, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv, t_dev);
+        e = md.model == 0 ? launch_pdl(k_tile_flip<0, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv)
+                          : launch_pdl(k_tile_flip<1, true>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv);
     else
-        e = md.model == 0 ? launch_pdl(k_tile_flip<0, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv, t_dev)
-                          : launch_pdl(k_tile_flip<1, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv, t_dev);
+        e = md.model == 0 ? launch_pdl(k_tile_flip<0, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv)
+                          : launch_pdl(k_tile_flip<1, false>, tiles, TILE_THREADS, stream, md, key, t, st.lab16, st.lab8, parent, st.ocount, in, out, st.bv);
     if (e != cudaSuccess) return -1;
     if (ev) cudaEventRecord(ev[3], stream);
     *launches += 3;
