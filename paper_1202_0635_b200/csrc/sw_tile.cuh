@@ -13,7 +13,7 @@
 //                 tile are marked open by their boundary sites, and the first thread to mark a root registers it as
 //                 node tile * OCAP + pos of the global union-find; B3b: the closed roots of all warps are listed
 //                 tile-wide and every thread draws one cluster decision per round (CLUSTER stream keyed on the root's
-//                 global site index); B4: every run resolves to its root.  Labels in shared memory are byte offsets
+//                 global site index); B4: every run resolves to its root.  Labels in shared memory are entry addresses
 //                 (a pointer hop is one LDS), the pointer in the low half of an entry, the output value in the high half.
 //        output   one byte per site: decision (closed cluster) or 16 + pos (open cluster) -- the low byte of the 16-bit
 //                 value DEC_BASE + decision / LOPEN | 16 + pos that tiles with many open roots write instead; the labels
@@ -142,26 +142,47 @@ static inline size_t tiled_workspace_bytes_n(int L, size_t nlat);
 static inline size_t tiled_workspace_bytes(int L) { return tiled_workspace_bytes_n(L, 1); }
 
 // ---- shared-memory union-find by minimum index (same scheme as uf_union in sw_generic.cuh) ------------------
-// Labels in shared memory are BYTE OFFSETS into the label array (4 x the skewed tile-local index): a hop is then one
-// LDS with the pointer as its address, no mask, no shift.  The low 16 bits of an entry hold the pointer (the entry's own
-// offset for a root), the high 16 bits stay 0 until the cluster's output value is known (phases B3, B3b).
-__device__ __forceinline__ uint32_t lab_ld(const char *lab, uint32_t off) { return *reinterpret_cast<const volatile uint32_t *>(lab + off); }
-__device__ __forceinline__ uint32_t ptr_ld(const char *lab, uint32_t off)
+// Labels in shared memory are the 32-bit SHARED-WINDOW ADDRESSES of label entries (base of the label array + 4 x the
+// skewed tile-local index; below 2^16): a hop is then one LDS with the pointer as its address, no mask, no shift, no add,
+// and the atomics take the address as it is.  The low 16 bits of an entry hold the pointer (the entry's own address for a
+// root), the high 16 bits stay 0 until the cluster's output value is known (phases B3, B3b).
+__device__ __forceinline__ uint32_t lab_ld(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t ptr_ld(uint32_t a)
 {
     // the 16-bit pointer field, zero-extended (PTX, so that the compiler keeps plain 32-bit compares on the result)
     uint32_t v;
-    asm volatile("ld.volatile.shared.u16 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(lab) + off) : "memory");
+    asm volatile("ld.volatile.shared.u16 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
     return v;
 }
-__device__ __forceinline__ void lab_st(char *lab, uint32_t off, uint32_t v) { *reinterpret_cast<volatile uint32_t *>(lab + off) = v; }
-
-__device__ __forceinline__ uint32_t sfind_halve(char *lab, uint32_t a)
+__device__ __forceinline__ void lab_st(uint32_t a, uint32_t v)
 {
-    uint32_t cur = lab_ld(lab, a);
+    asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t lab_min(uint32_t a, uint32_t v)
+{
+    uint32_t old;
+    asm volatile("atom.shared.min.u32 %0, [%1], %2;" : "=r"(old) : "r"(a), "r"(v) : "memory");
+    return old;
+}
+__device__ __forceinline__ uint32_t lab_or(uint32_t a, uint32_t v)
+{
+    uint32_t old;
+    asm volatile("atom.shared.or.b32 %0, [%1], %2;" : "=r"(old) : "r"(a), "r"(v) : "memory");
+    return old;
+}
+
+__device__ __forceinline__ uint32_t sfind_halve(uint32_t a)
+{
+    uint32_t cur = lab_ld(a);
     if (cur != a) {
         uint32_t prev = a, next;
-        while (cur > (next = lab_ld(lab, cur))) {
-            lab_st(lab, prev, next);
+        while (cur > (next = lab_ld(cur))) {
+            lab_st(prev, next);
             prev = cur;
             cur = next;
         }
@@ -169,14 +190,14 @@ __device__ __forceinline__ uint32_t sfind_halve(char *lab, uint32_t a)
     return cur;
 }
 
-__device__ __forceinline__ void sunion(char *lab, uint32_t a, uint32_t b)
+__device__ __forceinline__ void sunion(uint32_t a, uint32_t b)
 {
     for (;;) {
-        a = sfind_halve(lab, a);
-        b = sfind_halve(lab, b);
+        a = sfind_halve(a);
+        b = sfind_halve(b);
         if (a == b) return;
         if (a < b) { const uint32_t tmp = a; a = b; b = tmp; }
-        const uint32_t old = atomicMin(reinterpret_cast<uint32_t *>(lab + a), b);   // a > b
+        const uint32_t old = lab_min(a, b);   // a > b
         if (old == a) return;
         a = old;
     }
@@ -434,11 +455,11 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
     // ---------------- phase B: one thread per word --------------------------------------------------------
     // Label entries are addressed by SKEWED tile-local indices sp = p + (p >> 5) (one pad word per 32-site word), so that
     // the 32 lanes of a warp, which own 32 different words, hit 32 different banks when they touch the same bit position;
-    // what is stored and passed around is the BYTE OFFSET 4 sp of an entry (see lab_ld above).
-    char *const lab = reinterpret_cast<char *>(s_lab);
+    // what is stored and passed around is the shared-window ADDRESS sbase + 4 sp of an entry (see lab_ld above).
+    const uint32_t sbase = smem_u32(s_lab);
     constexpr uint32_t OPENBIT = 0x80000000u;                 // entry of a root of an open cluster (= LOPEN of its output value)
     const uint32_t wy = tid / NWORD, ww = tid % NWORD;
-    const uint32_t sb = 132u * tid;                           // offset of the entry of the word's first site
+    const uint32_t sb = sbase + 132u * tid;                   // address of the entry of the word's first site
     const uint32_t sbu = sb - 528u;                           // ... of the word above (tid - 4)
     const uint32_t h = s_H[wy][ww];
     const uint32_t hin = h & 0x7FFFFFFFu;                     // bonds inside the word
@@ -488,7 +509,7 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         uint32_t *el = s_edge[warp];
         for (uint32_t c = cs; c;) {
             const uint32_t k = pop_top(c);
-            lab_st(lab, sb + 4u * k, sb + 4u * k);
+            lab_st(sb + 4u * k, sb + 4u * k);
         }
         // `first` and the start bits of the runs that have an up-bond (S & ~cs) hold one bit per such run, in the same
         // order: both are walked from the top, so the run's start needs no search
@@ -497,7 +518,7 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
             const uint32_t bit = 1u << k;
             f ^= bit;
             fs ^= 1u << ks;
-            lab_st(lab, sb + 4u * ks, sbu + 4u * top_bit(Sa & (2u * bit - 1u)));
+            lab_st(sb + 4u * ks, sbu + 4u * top_bit(Sa & (2u * bit - 1u)));
         }
         for (uint32_t xr = X; xr;) {
             const uint32_t k = pop_top(xr);
@@ -525,18 +546,18 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
             bool have = e < ne;
             if (have) { const uint32_t v = s_edge[warp][e]; ea = v & 0xFFFFu; eb = v >> 16; }
             while (have) {
-                const uint32_t pa = lab_ld(lab, ea), pb = lab_ld(lab, eb);
-                const uint32_t ga = lab_ld(lab, pa), gb = lab_ld(lab, pb);
+                const uint32_t pa = lab_ld(ea), pb = lab_ld(eb);
+                const uint32_t ga = lab_ld(pa), gb = lab_ld(pb);
                 bool done = false;
                 if (pa != ea || pb != eb) {
-                    if (ga != pa) lab_st(lab, ea, ga);           // path halving: skip one ancestor on each side
-                    if (gb != pb) lab_st(lab, eb, gb);
+                    if (ga != pa) lab_st(ea, ga);           // path halving: skip one ancestor on each side
+                    if (gb != pb) lab_st(eb, gb);
                     ea = ga; eb = gb;
                 } else if (ea == eb) {
                     done = true;
                 } else {
                     const uint32_t hi = ea > eb ? ea : eb, lo = ea > eb ? eb : ea;
-                    const uint32_t old = atomicMin(reinterpret_cast<uint32_t *>(lab + hi), lo);
+                    const uint32_t old = lab_min(hi, lo);
                     if (old == hi) done = true;
                     else { ea = old; eb = lo; }                  // hi had a parent already: keep it connected to lo
                 }
@@ -552,10 +573,10 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
             uint32_t slot = epos0, Xr = X;
             while (Xr) {
                 const uint32_t k = pop_top(Xr);
-                if (slot >= (uint32_t)EDGE_CAP) sunion(lab, sb + 4u * seg_start(S, k), sbu + 4u * seg_start(Sa, k));
+                if (slot >= (uint32_t)EDGE_CAP) sunion(sb + 4u * seg_start(S, k), sbu + 4u * seg_start(Sa, k));
                 ++slot;
             }
-            if (hedge_out && slot >= (uint32_t)EDGE_CAP) sunion(lab, sb + 132u, sb + 4u * seg_start(S, 31u));
+            if (hedge_out && slot >= (uint32_t)EDGE_CAP) sunion(sb + 132u, sb + 4u * seg_start(S, 31u));
         }
     }
     __syncthreads();
@@ -569,32 +590,32 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         if (tid < (uint32_t)TW) {
             const uint32_t w = tid >> 5, k = tid & 31u;
             const uint32_t S0 = ~((s_H[0][w] & 0x7FFFFFFFu) << 1);
-            if ((S0 >> k) & 1u) c0 = 4u * (33u * w + k);
+            if ((S0 >> k) & 1u) c0 = sbase + 4u * (33u * w + k);
             const uint32_t hb = s_H[TH - 1][w] & 0x7FFFFFFFu, vb = s_V[TH - 1][w];
             const bool dup = k > 0u && ((vb & hb) >> (k - 1u)) & 1u;
-            if (((vb >> k) & 1u) && !dup) c1 = 4u * (33u * ((TH - 1) * NWORD + w) + seg_start(~(hb << 1), k));
+            if (((vb >> k) & 1u) && !dup) c1 = sbase + 4u * (33u * ((TH - 1) * NWORD + w) + seg_start(~(hb << 1), k));
         } else if (tid < (uint32_t)(TW + TH)) {
-            c0 = 4u * (33u * ((tid - TW) * NWORD));
+            c0 = sbase + 4u * (33u * ((tid - TW) * NWORD));
         } else if (tid < (uint32_t)(TW + 2 * TH)) {
             const uint32_t r = tid - (TW + TH);
             const uint32_t hr = s_H[r][NWORD - 1];
-            if (hr >> 31) c0 = 4u * (33u * (r * NWORD + NWORD - 1) + seg_start(~((hr & 0x7FFFFFFFu) << 1), 31u));
+            if (hr >> 31) c0 = sbase + 4u * (33u * (r * NWORD + NWORD - 1) + seg_start(~((hr & 0x7FFFFFFFu) << 1), 31u));
         }
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
             uint32_t a = c ? c1 : c0;
             if (a != 0xFFFFFFFFu) {
                 uint32_t p;
-                while ((p = ptr_ld(lab, a)) != a) a = p;
+                while ((p = ptr_ld(a)) != a) a = p;
                 // The first thread to mark a root registers it: node blockIdx.x * OCAP + pos of the global union-find, its
                 // own parent, key = (site, node); the root's entry gets its output value LOPEN | pos in the upper half.
                 // (Atomic ORs: other boundary sites of the cluster mark the same entry at the same time.)
-                const uint32_t old = atomicOr(reinterpret_cast<uint32_t *>(lab + a), OPENBIT);
+                const uint32_t old = lab_or(a, OPENBIT);
                 if (!(old & OPENBIT)) {
                     const uint32_t pos = atomicAdd(&s_nopen, 1u);
                     const uint32_t node = blockIdx.x * (uint32_t)OCAP + pos;
-                    parent[node] = ((unsigned long long)root_site(a >> 2, x0, y0, L) << 32) | node;
-                    atomicOr(reinterpret_cast<uint32_t *>(lab + a), (POS_BASE + pos) << 16);
+                    parent[node] = ((unsigned long long)root_site((a - sbase) >> 2, x0, y0, L) << 32) | node;
+                    lab_or(a, (POS_BASE + pos) << 16);
                 }
             }
         }
@@ -634,13 +655,13 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
             cand &= ~ax;
             while (ax) {                          // (also when B3 marked it open: it has no bond at all, so it is closed)
                 const uint32_t k = pop_top(ax);
-                lab_st(lab, sb + 4u * k, (sb + 4u * k) | ((fuse ? (uint32_t)DEC_BASE : (sb >> 2) + k) << 16));
+                lab_st(sb + 4u * k, (sb + 4u * k) | ((fuse ? (uint32_t)DEC_BASE : ((sb - sbase) >> 2) + k) << 16));
             }
         }
         if (wy == 0u) cand = 0u;                  // every cluster with a site in the top row is open
         for (uint32_t c = cand; c;) {
             const uint32_t k = pop_top(c);
-            if (lab_ld(lab, sb + 4u * k) == sb + 4u * k) rall |= 1u << k;     // a root, and not open (upper half still 0)
+            if (lab_ld(sb + 4u * k) == sb + 4u * k) rall |= 1u << k;     // a root, and not open (upper half still 0)
         }
         // The closed roots of all warps go to one tile-wide list (16-bit entries in the storage of the edge lists, which
         // B2 has left), so that after the barrier every thread takes one root per round and all warps carry the same
@@ -664,8 +685,8 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
     }
     __syncthreads();
     {
-        auto decide = [&](uint32_t o) {           // o = offset of the entry of a closed root
-            const uint32_t sp = o >> 2;
+        auto decide = [&](uint32_t o) {           // o = address of the entry of a closed root
+            const uint32_t sp = (o - sbase) >> 2;
             uint32_t out = sp;
             if (fuse) {
                 const uint32_t r = root_site(sp, x0, y0, L);
@@ -674,7 +695,7 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
                 const uint32_t wsel = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
                 out = (uint32_t)DEC_BASE + (MODEL == 0 ? mulhi_q(wsel, (uint32_t)md.q) : (wsel >> 31));
             }
-            lab_st(lab, o, o | (out << 16));
+            lab_st(o, o | (out << 16));
         };
         const uint32_t nc0 = s_nroot, nc = nc0 < (uint32_t)RLCAP ? nc0 : (uint32_t)RLCAP;
         for (uint32_t i = tid; i < nc; i += TILE_THREADS) decide(rl[i]);
@@ -700,11 +721,11 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
                 const uint32_t k0 = (uint32_t)__ffs((int)todo) - 1u, k1 = top_bit(todo);
                 todo &= todo - 1u;
                 todo &= ~(1u << k1);
-                uint32_t x0 = ptr_ld(lab, sb + 4u * k0), x1 = ptr_ld(lab, sb + 4u * k1);
-                x0 = ptr_ld(lab, x0); x1 = ptr_ld(lab, x1);
-                const uint32_t y0r = lab_ld(lab, x0), y1r = lab_ld(lab, x1);
-                lab_st(lab, sb + 4u * k0, y0r);
-                lab_st(lab, sb + 4u * k1, y1r);
+                uint32_t x0 = ptr_ld(sb + 4u * k0), x1 = ptr_ld(sb + 4u * k1);
+                x0 = ptr_ld(x0); x1 = ptr_ld(x1);
+                const uint32_t y0r = lab_ld(x0), y1r = lab_ld(x1);
+                lab_st(sb + 4u * k0, y0r);
+                lab_st(sb + 4u * k1, y1r);
                 if ((y0r ^ x0) & 0xFFFCu) rem |= 1u << k0;         // pointer fields differ (offsets are multiples of 4)
                 if ((y1r ^ x1) & 0xFFFCu) rem |= 1u << k1;
             }
@@ -716,9 +737,9 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         while (rem) {
             const uint32_t k = top_bit(rem);
             rem ^= 1u << k;
-            uint32_t a = ptr_ld(lab, sb + 4u * k), p;
-            while ((p = ptr_ld(lab, a)) != a) { a = p; ++hops; }
-            lab_st(lab, sb + 4u * k, lab_ld(lab, a));
+            uint32_t a = ptr_ld(sb + 4u * k), p;
+            while ((p = ptr_ld(a)) != a) { a = p; ++hops; }
+            lab_st(sb + 4u * k, lab_ld(a));
         }
     }
     __syncwarp();
@@ -731,7 +752,7 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         if (tid == 0u) ocount[blockIdx.x] = nopen | (narrow ? 0u : WIDE_FLAG);
         uint32_t xs[32];
 #pragma unroll
-        for (int k = 0; k < 32; ++k) xs[k] = ((S >> k) & 1u) ? lab_ld(lab, sb + 4u * k) : 0u;
+        for (int k = 0; k < 32; ++k) xs[k] = ((S >> k) & 1u) ? lab_ld(sb + 4u * k) : 0u;
         uint16_t *ed = edges + (size_t)blockIdx.x * ECNT;       // the labels of the tile's boundary sites, compact, for K2
         const bool edge_row = wy == 0u || wy == (uint32_t)TH - 1u;
         uint32_t cur = 0u;
