@@ -231,7 +231,7 @@ int generic_sweep(sw_ctx *c, uint32_t t, cudaEvent_t *ev)
 
 // obs_row (optional): zeroed row of the record ring that receives the observables of S^t if the back-end fuses S5 into
 // its first kernel (fuses_observables); otherwise the caller has launched k_observables on it already.
-bool fuses_observables(const sw_ctx *c) { return c->algo == SW_ALGO_TILED && sw::tiled_fuses_observables(c->md); }
+bool fuses_observables(const sw_ctx *c) { return c->algo == SW_ALGO_TILED && !c->stats_on && sw::tiled_fuses_observables(c->md); }
 
 // sw_sweep(n) of the tiled back-end, n >= GRAPH_SWEEPS: the 3 kernels of GRAPH_SWEEPS consecutive sweeps (with their
 // programmatic-dependent-launch edges) are captured once per ping-pong parity and replayed with one cudaGraphLaunch per

@@ -275,7 +275,9 @@ __global__ void k_selftest_compare(const uint32_t *vals, int n, int *bad)
 // through plain loads issued while the box is in flight.
 // BATCH: blockIdx.x is a global tile of a batch (BatchView above); the lattice's Philox key then lives in registers
 // instead of the constant bank, which costs the fifth resident CTA.
-template <int MODEL, bool OBS, bool BATCH>
+// STATS: the work counters and per-phase clocks of sw_stats (an instantiation of its own: the production kernel carries
+// neither the tests nor the two registers of the phase clock).
+template <int MODEL, bool OBS, bool BATCH, bool STATS = false>
 __global__ void __launch_bounds__(TILE_THREADS, BATCH ? 4 : SW_LABEL_MINB)
 k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, const __grid_constant__ CUtensorMap spin_map,
              uint16_t *lab16, uint8_t *lab8, unsigned long long *parent, uint32_t *hedge, uint32_t *vedge, uint16_t *edges, uint32_t *ocount,
@@ -325,9 +327,10 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
     }
     const PhiloxKey &key = BATCH ? key_lat : key_one;
     // per-phase clocks (lane 0 of every warp), only when the work counters are on: stats[8 + phase]
-    long long ph_t = stats ? clock64() : 0;
+    long long ph_t = STATS ? clock64() : 0;
+    (void)ph_t;
 #define SW_PHASE(i)                                                                     \
-    if (stats) {                                                                        \
+    if (STATS) {                                                                        \
         const long long now_ = clock64();                                               \
         if (lane == 0u) atomicAdd(stats + 8 + (i), (unsigned long long)(now_ - ph_t)); \
         ph_t = now_;                                                                    \
@@ -795,7 +798,7 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         if (ww == 0u) ed[wy] = (uint16_t)((xs[0] >> 16) & emask);
         if (ww == (uint32_t)NWORD - 1u) ed[TH + wy] = (uint16_t)((cur >> 16) & emask);
         SW_PHASE(6)
-        if (stats) {
+        if (STATS) {
             const uint32_t n2 = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popc(S));
             const uint32_t n3 = __reduce_add_sync(0xFFFFFFFFu, epos - epos0);
             const uint32_t n4 = __reduce_add_sync(0xFFFFFFFFu, hops);
@@ -1118,6 +1121,13 @@ static inline cudaError_t tiled_launch_label(TiledState &st, const Model &md, co
                               st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
         return launch_pdl(k_tile_label<1, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
                           st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+    }
+    if (stats && !st.batch) {          // counters on: the STATS instantiation (the caller does not fuse observables then)
+        if (md.model == 0)
+            return launch_pdl(k_tile_label<0, false, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent,
+                              st.hedge, st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
+        return launch_pdl(k_tile_label<1, false, false, true>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent,
+                          st.hedge, st.vedge, st.edges, st.ocount, fuse, stats, none, st.bv);
     }
     if (md.model == 0 && md.q == 2 && obs)
         return launch_pdl(k_tile_label<0, true, false>, tiles, TILE_THREADS, stream, md, key, t, in, tm, st.lab16, st.lab8, parent, st.hedge,
