@@ -571,15 +571,31 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
                 }
             }
         }
-        if (etotal > (uint32_t)EDGE_CAP && epos > (uint32_t)EDGE_CAP) {
-            // rare: the list overflowed; this thread unions its unlisted edges itself
-            uint32_t slot = epos0, Xr = X;
+        if (etotal > (uint32_t)EDGE_CAP) {
+            // rare (warp-uniform): the list overflowed; every thread unions its unlisted edges itself.  Everything is
+            // computed again from the masks in shared memory, so that the common path keeps no register for this one.
+            const uint32_t u2 = wy > 0u ? s_V[wy - 1][ww] : 0u;
+            const uint32_t ha2 = wy > 0u ? s_H[wy - 1][ww] & 0x7FFFFFFFu : 0u;
+            const uint32_t Sa2 = ~(ha2 << 1);
+            const uint32_t g2 = u2 & hin, sum2 = hin + g2;
+            const uint32_t first2 = (g2 & (sum2 ^ hin)) | (u2 & ~hin & ~sum2);
+            const uint32_t C2 = ha2 & hin, gC2 = u2 & C2;
+            uint32_t Xr = u2 & ~first2 & ~((C2 + gC2) ^ C2 ^ gC2);
+            const bool hedge2 = (ww + 1u < (uint32_t)NWORD) && (h >> 31);
+            const uint32_t n2 = __popc(Xr) + (hedge2 ? 1u : 0u);
+            uint32_t incl2 = n2;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl2, d);
+                if (lane >= (uint32_t)d) incl2 += o;
+            }
+            uint32_t slot = incl2 - n2;                         // the slots are taken in the order of B1's loop
             while (Xr) {
                 const uint32_t k = pop_top(Xr);
-                if (slot >= (uint32_t)EDGE_CAP) sunion(sb + 4u * seg_start(S, k), sbu + 4u * seg_start(Sa, k));
+                if (slot >= (uint32_t)EDGE_CAP) sunion(sb + 4u * seg_start(S, k), sbu + 4u * seg_start(Sa2, k));
                 ++slot;
             }
-            if (hedge_out && slot >= (uint32_t)EDGE_CAP) sunion(sb + 132u, sb + 4u * seg_start(S, 31u));
+            if (hedge2 && slot >= (uint32_t)EDGE_CAP) sunion(sb + 132u, sb + 4u * seg_start(S, 31u));
         }
     }
     __syncthreads();
