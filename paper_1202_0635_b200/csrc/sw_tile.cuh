@@ -770,8 +770,10 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
         const bool narrow = fuse && nopen <= NARROW_MAX;
         if (tid == 0u) ocount[blockIdx.x] = nopen | (narrow ? 0u : WIDE_FLAG);
         uint32_t xs[32];
+        uint32_t sbr = sb;                        // pinned in a register: else the address is rebuilt for every predicated load
+        asm volatile("" : "+r"(sbr));
 #pragma unroll
-        for (int k = 0; k < 32; ++k) xs[k] = ((S >> k) & 1u) ? lab_ld(sb + 4u * k) : 0u;
+        for (int k = 0; k < 32; ++k) xs[k] = ((S >> k) & 1u) ? lab_ld(sbr + 4u * k) : 0u;
         uint16_t *ed = edges + (size_t)blockIdx.x * ECNT;       // the labels of the tile's boundary sites, compact, for K2
         const bool edge_row = wy == 0u || wy == (uint32_t)TH - 1u;
         uint32_t cur = 0u;
