@@ -116,6 +116,19 @@ def test_tiled_equals_generic_on_device(sw):
             assert np.array_equal(a.get_labels(), b.get_labels())
 
 
+@pytest.mark.parametrize("L,q,model,T,n", [(1024, 2, POTTS, tc(2), 6000), (512, 6, CLOCK, 0.9, 6000), (1024, 2, POTTS, 0.8 * tc(2), 4000)])
+def test_soak_tiled_graph_path_equals_generic(sw, L, q, model, T, n):
+    """Thousands of sweeps through the CUDA-graph replay of the tiled back-end against the generic back-end (races in the
+    shared-memory union-find or in the seam merge would show up as a diverging trajectory sooner or later)."""
+    with sw.Lattice(L, q, model, T, 4242, algo=TILED) as a, sw.Lattice(L, q, model, T, 4242, algo=GENERIC) as b:
+        for k in range(n // 1000):
+            a.sweep(1000)
+            b.sweep(1000)
+            assert np.array_equal(a.get_spins(), b.get_spins()), k
+        assert np.array_equal(a.get_labels(), b.get_labels())
+        assert a.stats()[7] > 0
+
+
 @pytest.mark.parametrize("L,q,model,T", [(256, 2, POTTS, tc(2)), (384, 6, CLOCK, 0.9)])
 def test_graph_replay_equals_plain_launches_and_the_oracle(sw, oracle, L, q, model, T):
     """sw_sweep(n >= 16) of the tiled back-end replays chunks of 16 sweeps from a CUDA graph whose kernel nodes get their sweep
