@@ -933,11 +933,14 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
 }
 
 // K3.  grid = tiles, block = TILE_THREADS; 32 sites per thread (4 passes of 8).  in = S^t, out = S^{t+1}.
+// Resident CTAs per SM: 8 (all 2048 threads) for the Potts kernel -- no difference while the labels sit in L2 (L <= 4096), but
+// beyond that the kernel streams from HBM and every tile first waits for the chase of its open roots: 183 -> 140 us at
+// L = 16384; the clock kernel keeps more registers (old spins in flight) and stops at 6.
 #ifndef SW_FLIP_MINB
-#define SW_FLIP_MINB 1
+#define SW_FLIP_MINB(MODEL, BATCH) ((BATCH) ? 4 : (MODEL) == 0 ? 8 : 6)
 #endif
 template <int MODEL, bool BATCH>
-__global__ void __launch_bounds__(TILE_THREADS, SW_FLIP_MINB)
+__global__ void __launch_bounds__(TILE_THREADS, SW_FLIP_MINB(MODEL, BATCH))
 k_tile_flip(Model md, PhiloxKey key_one, uint32_t t, const uint16_t *lab16, const uint8_t *lab8, unsigned long long *parent, const uint32_t *ocount,
             const uint8_t *in, uint8_t *out, BatchView bv)
 {
