@@ -730,8 +730,8 @@ k_tile_label(Model md, PhiloxKey key_one, uint32_t t, const uint8_t *spins, cons
 
     SW_PHASE(7)
     // B4a: resolve every run of the word to its root's entry (whose upper half is the output value).  Two runs at
-    // a time, three pointer hops each (the loads of one level are independent, so their latencies overlap; the first two
-    // read the 16-bit pointer only), result written back to the run's own entry; runs deeper than that (rare) are
+    // a time, SW_RESOLVE_HOPS pointer hops each (the loads of one level are independent, so their latencies overlap; all but
+    // the last read the 16-bit pointer only), result written back to the run's own entry; runs deeper than that (rare) are
     // finished by a chase that starts from the already advanced pointer.
     uint32_t hops = 0u;
     {
