@@ -900,7 +900,9 @@ k_seam_merge(Model md, const uint32_t *hedge, const uint32_t *vedge, const uint1
     const uint32_t L = (uint32_t)md.L;
     const uint32_t tiles_x = L / TW, tiles_y = L / TH;
     const uint32_t nh = tiles_x * L, ne = nh + tiles_y * L;
-    uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+    // blocks take the positions in reverse order (bottom edges of the lowest tiles first): measured 0.5-1 us faster per
+    // sweep than the forward order at L=4096 (the union order shapes the chains that K2 and K3 have to walk)
+    uint32_t e = (gridDim.x - 1u - blockIdx.x) * blockDim.x + threadIdx.x;
     pdl_prologue();
     if (e >= ne * nlat) return;
     const uint32_t lat = e / ne;          // ne is a multiple of 32: uniform in a warp
