@@ -225,6 +225,30 @@ const char *sw_microbench_name(int probe);
  * toolchain's carry convention differs from the one the kernels were written for (every clock bond would flip). */
 int sw_selftest(void);
 
+/* One sweep WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): no context, no workspace argument.  The scratch of the sweep (clock threshold
+ * table, bonds S1, union-find parents S2: 4096 + 5 * SW_NOALLOC_MAX_L^2 bytes = 5 MiB + 4 KiB) is a file-scope
+ * `static __device__` array of libsw.so; every GPU that loads the library holds it until the process exits.
+ *   d_spins_out = the configuration sweep `sweep_index` (S1..S4 of the generic back-end) makes of
+ *   d_spins_in, bit for bit what sw_create(L, q, model, T, seed); sw_set_spins(in, sweep_index); sw_sweep(1);
+ *   sw_get_spins(out) gives with any back-end.
+ * d_spins_in, d_spins_out: DEVICE memory of the current device, L*L bytes each, row-major, owned by the caller;
+ * they may be the same buffer but must not overlap partially.  Values >= q are NOT checked (the result is then
+ * unspecified, but no access leaves the scratch or the two buffers).  cuda_stream: a cudaStream_t of the current
+ * device, or NULL for the default stream.  The call is ASYNCHRONOUS: it enqueues one small copy (clock model only, the
+ * threshold table, from host stack memory) and 5 kernels on the stream and returns; synchronise the stream before
+ * reading d_spins_out.  It calls no cudaMalloc, cudaFree or allocating library routine; the address of the scratch is
+ * taken once per device with cudaGetSymbolAddress.
+ * Limits: 2 <= L <= SW_NOALLOC_MAX_L (larger L: SW_ERR_UNSUPPORTED, nothing enqueued), q, T, model as for sw_create,
+ * sweep_index <= 2^32-1.
+ * Every call on a device shares the one scratch array, which keeps the previous call's contents: each call rewrites
+ * all of it that it reads (nothing has to start at zero), and calls are ordered only by their streams -- two calls
+ * that overlap on the GPU (different streams, or different host threads on different streams) RACE on the scratch and
+ * give garbage.  Calls on the same stream, or otherwise ordered, are safe. */
+#define SW_NOALLOC_MAX_L 1024
+int sw_sweep_noalloc(int L, int q, int model, double T, uint64_t seed, uint64_t sweep_index,
+                     const uint8_t *d_spins_in, uint8_t *d_spins_out, void *cuda_stream);
+
 /* Thread-local description of the last failure in this thread ("" if none). */
 const char *sw_last_error(void);
 

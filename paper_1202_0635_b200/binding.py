@@ -80,6 +80,7 @@ SYMBOLS = {
     "sw_microbench": (_i, [_i, _i, _i, _vp]),
     "sw_microbench_name": (ctypes.c_char_p, [_i]),
     "sw_selftest": (_i, []),
+    "sw_sweep_noalloc": (_i, [_i, _i, _i, _d, _u64, _u64, _vp, _vp, _vp]),
     "sw_last_error": (ctypes.c_char_p, []),
 }
 
@@ -320,6 +321,21 @@ class Batch:
     @property
     def sweep_index(self) -> int:
         return int(self._lib.sw_batch_sweep_index(self._h))
+
+
+SW_NOALLOC_MAX_L = 1024
+
+
+def sweep_noalloc(L: int, q: int, model: int, T: float, seed: int, sweep_index: int, d_spins_in, d_spins_out, stream=None):
+    """sw_sweep_noalloc: one sweep from/to DEVICE buffers (torch CUDA uint8 tensors or raw device pointers), scratch in
+    the library's static device array, no allocation.  Asynchronous on `stream` (a raw cudaStream_t, default: torch's
+    current stream); synchronise before reading the output."""
+    def dev_ptr(a):
+        return int(a) if isinstance(a, int) else a.data_ptr()
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    _check(load().sw_sweep_noalloc(L, q, model, float(T), seed, sweep_index, dev_ptr(d_spins_in), dev_ptr(d_spins_out), stream))
 
 
 # Derived doubles (DESIGN.md R11, R15): computed by libsw.so (sw_derive_*), marshalled here.

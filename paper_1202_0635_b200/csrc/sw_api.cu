@@ -1051,3 +1051,149 @@ int sw_selftest(void)
 const char *sw_last_error(void) { return g_err; }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// sw_sweep_noalloc (include/sw.h): one sweep of the generic back-end whose scratch is a static device array, for callers
+// that cannot call cudaMalloc.  No existing path uses anything below.
+// ---------------------------------------------------------------------------------------------------------------------
+#include <mutex>
+
+namespace {
+
+constexpr size_t NOALLOC_MAX_N = (size_t)SW_NOALLOC_MAX_L * SW_NOALLOC_MAX_L;
+constexpr size_t NOALLOC_TABLE_BYTES = 4 * (size_t)(2 * SW_MAX_Q) * (2 * SW_MAX_Q);   // 4096: clock thresholds, (2q)^2 words
+constexpr size_t NOALLOC_LABELS_OFF = NOALLOC_TABLE_BYTES;                            // int32 parents, 4 bytes per site
+constexpr size_t NOALLOC_BONDS_OFF = NOALLOC_LABELS_OFF + 4 * NOALLOC_MAX_N;          // bond bits, 1 byte per site
+constexpr size_t NOALLOC_BYTES = NOALLOC_BONDS_OFF + NOALLOC_MAX_N;                   // 5 MiB + 4 KiB
+
+}  // namespace
+
+// The scratch.  In HOST code this name is only a stand-in for the symbol (not a device address): the host takes the
+// address once per device with cudaGetSymbolAddress (noalloc_scratch) and hands that pointer to the kernels.
+// The table comes first: a threshold lookup with an (unchecked) spin value >= q lands at most
+// 4 * ((2*255 + 2q)*2q + 2*255 + 2q) < 72 KB past its start, inside the array.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_BYTES];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+unsigned char *g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};   // device address of g_noalloc_scratch, per device ordinal
+
+// The device address of the scratch on the CURRENT device (looked up on the first call per device, with that device current).
+int noalloc_scratch(int dev, unsigned char **out)
+{
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void *p = nullptr;
+        CU_TRY(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        if (!p) return fail(SW_ERR_CUDA, "sw_sweep_noalloc: cudaGetSymbolAddress returned NULL on device %d", dev);
+        g_noalloc_ptr[dev] = static_cast<unsigned char *>(p);
+    }
+    *out = g_noalloc_ptr[dev];
+    return SW_OK;
+}
+
+// The thresholds of build_thresholds (R1, R4, R6), written to caller storage without touching the heap:
+// Potts -> out[0]; clock -> out[ci * 2q + cj].
+void noalloc_thresholds(int model, int q, double T, uint32_t *out)
+{
+    if (model == SW_POTTS) {
+        out[0] = thr_from_p(1.0 - std::exp(-1.0 / T));
+        return;
+    }
+    const int n = 2 * q;
+    const double pi = 3.14159265358979323846;
+    double s[2 * SW_MAX_Q];
+    for (int k = 0; k < n; ++k) s[k] = (k % q == 0) ? 0.0 : std::sin(pi * (double)k / (double)q);
+    for (int a = 0; a < n; ++a)
+        for (int b = 0; b < n; ++b) {
+            const double pr = s[a] * s[b];
+            out[(size_t)a * n + b] = pr > 0.0 ? thr_from_p(1.0 - std::exp(-2.0 * pr / T)) : 0u;
+        }
+}
+
+// S3 + S4 as sw::k_flip computes them, from `in` to `out` (which may be the same buffer: a thread reads and writes its own site only)
+__global__ void k_flip_io(sw::Model md, sw::PhiloxKey key, uint32_t t, const int32_t *__restrict__ labels, const uint8_t *in, uint8_t *out)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= md.N) return;
+    const uint32_t r = (uint32_t)labels[i];
+    uint32_t w[4];
+    sw::philox_stream<sw::STREAM_CLUSTER>(key, r >> 2, t, w);
+    const uint32_t ww = (r & 2u) ? ((r & 1u) ? w[3] : w[2]) : ((r & 1u) ? w[1] : w[0]);
+    const uint32_t s = in[i];
+    uint32_t v = s;
+    if (md.model == 0) {
+        v = sw::mulhi_q(ww, (uint32_t)md.q);
+    } else if (ww >> 31) {
+        const uint32_t m = sw::axis_of_sweep(key, t, (uint32_t)md.q);
+        v = m + (uint32_t)md.q - s;          // in (0, 2q) for s < q
+        if (v >= (uint32_t)md.q) v -= (uint32_t)md.q;
+    }
+    out[i] = (uint8_t)v;
+}
+
+// device memory of device `dev` (cudaPointerGetAttributes allocates nothing)
+bool noalloc_on_device(const void *p, int dev)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return (a.type == cudaMemoryTypeDevice && a.device == dev) || a.type == cudaMemoryTypeManaged;
+}
+
+}  // namespace
+
+extern "C" int sw_sweep_noalloc(int L, int q, int model, double T, uint64_t seed, uint64_t sweep_index,
+                                const uint8_t *d_spins_in, uint8_t *d_spins_out, void *cuda_stream)
+{
+    if (L > SW_NOALLOC_MAX_L)
+        return fail(SW_ERR_UNSUPPORTED, "sw_sweep_noalloc: L = %d exceeds SW_NOALLOC_MAX_L = %d (the static scratch of %zu bytes holds "
+                    "5 bytes per site of a %d x %d lattice); use sw_create / sw_create_in for larger lattices",
+                    L, SW_NOALLOC_MAX_L, NOALLOC_BYTES, SW_NOALLOC_MAX_L, SW_NOALLOC_MAX_L);
+    if (!args_ok(L, q, model) || !(T > 0.0) || !std::isfinite(T))
+        return fail(SW_ERR_ARG, "sw_sweep_noalloc: need 2<=L<=%d, 2<=q<=%d, model in {0,1}, finite T>0 (got L=%d q=%d model=%d T=%g)",
+                    SW_NOALLOC_MAX_L, SW_MAX_Q, L, q, model, T);
+    if (sweep_index > 0xFFFFFFFFull) return fail(SW_ERR_ARG, "sw_sweep_noalloc: sweep index must fit 32 bits");
+    if (!d_spins_in || !d_spins_out) return fail(SW_ERR_ARG, "sw_sweep_noalloc: NULL spin buffer");
+    const size_t N = (size_t)L * (size_t)L;
+    if (d_spins_in != d_spins_out && d_spins_in < d_spins_out + N && d_spins_out < d_spins_in + N)
+        return fail(SW_ERR_ARG, "sw_sweep_noalloc: d_spins_in and d_spins_out overlap partially");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(SW_ERR_CUDA, "sw_sweep_noalloc: no usable CUDA device (this library has no CPU fallback)");
+    }
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(SW_ERR_UNSUPPORTED, "sw_sweep_noalloc: device ordinal %d not below %d", dev, NOALLOC_MAX_DEVICES);
+    if (!noalloc_on_device(d_spins_in, dev) || !noalloc_on_device(d_spins_out, dev))
+        return fail(SW_ERR_ARG, "sw_sweep_noalloc: d_spins_in / d_spins_out must be device memory of the current device (%d)", dev);
+    unsigned char *scratch = nullptr;
+    int rc = noalloc_scratch(dev, &scratch);
+    if (rc != SW_OK) return rc;
+
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    uint32_t *table = reinterpret_cast<uint32_t *>(scratch);
+    int32_t *labels = reinterpret_cast<int32_t *>(scratch + NOALLOC_LABELS_OFF);
+    uint8_t *bonds = scratch + NOALLOC_BONDS_OFF;
+
+    uint32_t thr[(2 * SW_MAX_Q) * (2 * SW_MAX_Q)];
+    noalloc_thresholds(model, q, T, thr);
+    sw::Model md{};
+    md.L = L; md.q = q; md.model = model; md.N = (uint32_t)N;
+    md.thr_potts = model == SW_POTTS ? thr[0] : 0u;
+    md.table = table;
+    // pageable host memory: the copy is staged before cudaMemcpyAsync returns, so `thr` may leave scope
+    if (model == SW_CLOCK) CU_TRY(cudaMemcpyAsync(table, thr, 4 * (size_t)(2 * q) * (2 * q), cudaMemcpyHostToDevice, stream));
+    const sw::PhiloxKey key = sw::make_philox_key(seed);
+    const uint32_t t = (uint32_t)sweep_index;
+    const unsigned bs = 256;
+    // every byte of the scratch these kernels read is written here first (labels by k_label_init, bonds by k_bonds,
+    // the table by the copy above): whatever the previous call left behind is never seen
+    sw::k_bonds<<<blocks_for((N + 1) / 2, bs), bs, 0, stream>>>(md, key, t, d_spins_in, bonds);
+    sw::k_label_init<<<blocks_for(N, bs), bs, 0, stream>>>(md.N, labels);
+    sw::k_union<<<blocks_for(N, bs), bs, 0, stream>>>(md, bonds, labels);
+    sw::k_flatten<<<blocks_for(N, bs), bs, 0, stream>>>(md.N, labels);
+    k_flip_io<<<blocks_for(N, bs), bs, 0, stream>>>(md, key, t, labels, d_spins_in, d_spins_out);
+    CU_TRY(cudaGetLastError());
+    return SW_OK;
+}
